@@ -115,12 +115,16 @@ def test_taylor_green_vortex_decay(oracle_mod):
 
 
 def test_rk3_temporal_order(oracle_mod):
-    """Wray's low-storage RK3 (N1): gamma = 8/15, 5/12, 3/4, zeta = 0, -17/60, -5/12.  With the
-    projection applied at every substep the velocity/phase field converge at order >= 2 in dt
-    (self-convergence, matched density so that the pressure splitting is exact).  Wrong
-    coefficients (e.g. sum alpha != 1 or a swapped zeta) drop the order to <= 1."""
+    """Wray's low-storage RK3 (N1): gamma = 8/15, 5/12, 3/4, zeta = 0, -17/60, -5/12.  With
+    matched properties and sigma = 0 the velocity does not feel phi, the pressure splitting is
+    exact and the projection commutes with the periodic operators, so u follows a plain RK3
+    integration of the projected ODE (order 3) and phi a consistent RK3 with the stage
+    velocities (order 3).  Wrong coefficients (sum alpha != 1, a swapped zeta, a wrong
+    alpha in the Poisson rhs) drop the order to <= 1-2.
+    (With sigma != 0 the sequential update of N6 -- S3 sees phi_new -- makes the phi-u
+    coupling first order in dt; measured 1.0, recorded in DESIGN.md.)"""
     cfg, f, dt0, _ = W.make(1, grid=(16, 16, 16), ndrops=2, radius=0.9)
-    cfg.update(mu1=0.02, mu2=0.02, gamma_rel=0.0, gamma_abs=1.2)
+    cfg.update(mu1=0.02, mu2=0.02, gamma_rel=0.0, gamma_abs=1.2, sigma=0.0)
     T = 0.16
 
     def run(nsteps):
@@ -133,4 +137,4 @@ def test_rk3_temporal_order(oracle_mod):
     a, b, c = run(4), run(8), run(16)
     for k in ("u", "v", "phi"):
         e1, e2 = np.abs(a[k] - b[k]).max(), np.abs(b[k] - c[k]).max()
-        assert math.log2(e1 / e2) > 1.8, (k, e1, e2)
+        assert math.log2(e1 / e2) > 2.7, (k, e1, e2, math.log2(e1 / e2))

@@ -1,0 +1,134 @@
+/* fizzy.h -- C ABI of libfizzy.so: one low-storage RK3 substep of the CaNS-Fizzy one-fluid
+ * two-phase solver (arXiv 2502.04189) on one NVIDIA B200 (sm_100a), fp64.
+ *
+ * What the library computes (passages: /root/reference/PAPER.md, cited PAPER.md:<line>;
+ * formulas (i)-(v) of BASELINE.json:5 `north_star`; discrete readings N1..N22 in DESIGN.md):
+ *   PAPER.md:32 (section 2)  one-fluid model: incompressible Navier-Stokes + heat transport +
+ *                            ACDI phase-field transport; properties mapped linearly over phi;
+ *                            CSF surface tension.
+ *   PAPER.md:36 (section 3)  2nd-order finite differences, staggered velocity / cell-centred
+ *                            scalars; low-storage three-step Runge-Kutta; pressure correction with
+ *                            the Dong-Shen / Dodd-Ferrante splitting -> constant-coefficient
+ *                            Poisson equation solved by the FFT direct solver of CaNS; mass-
+ *                            momentum consistent regularisation flux in the momentum equation.
+ *
+ * Layout.  Every field is nx*ny*nz contiguous doubles, x fastest: idx = i + nx*(j + ny*k).
+ * u[i,j,k] sits on the x-face between cells i and i+1, v on the y-face between j and j+1,
+ * w on the z-face zf[k+1] between cells k and k+1.  x and y are periodic.  z is periodic
+ * (z_wall = 0) or bounded by no-slip walls (z_wall = 1; then w[:,:,nz-1] == 0 always).
+ * Fluid 1 <-> phi = 1 (dispersed), fluid 2 <-> phi = 0 (carrier).
+ *
+ * Pointers.  Field pointers given to fizzy_set_fields / fizzy_get_fields / fizzy_poisson_solve
+ * may be DEVICE pointers or HOST pointers (pinned or pageable; the copy is a
+ * cudaMemcpyAsync(cudaMemcpyDefault) on the context's stream).  `zf` in fizzy_grid is a HOST
+ * pointer.  `dev_workspace` is a DEVICE pointer.  The caller owns every buffer it passes; the
+ * library owns only the opaque context (host memory) and never calls cudaMalloc for fields.
+ *
+ * Execution.  All calls enqueue work on the stream given at creation and return without
+ * synchronising, except fizzy_gamma (reads one double back) and calls that copy to pageable
+ * host memory (CUDA semantics).  No exceptions cross the ABI, no aborts, no global state.
+ * There is no CPU fallback: without a CUDA device fizzy_create returns FIZZY_ECUDA.
+ */
+#ifndef FIZZY_H
+#define FIZZY_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct fizzy_ctx fizzy_ctx; /* opaque, owned by the library */
+
+typedef enum {
+    FIZZY_OK = 0,
+    FIZZY_EINVAL = 1, /* bad argument (see each call) */
+    FIZZY_ENOMEM = 2, /* workspace too small / host allocation failed */
+    FIZZY_ECUDA = 3,  /* CUDA runtime error; text via fizzy_last_error */
+    FIZZY_ESTATE = 4  /* call out of order (substep before set_fields, stage sequence) */
+} fizzy_status;
+
+/* Grid ("3D Cartesian grid").  nx, ny powers of two in [8, 1024]; nz >= 4.
+ * zf == NULL: uniform z.  Otherwise nz+1 HOST doubles, zf[0] = 0, zf[nz] = lz, strictly
+ * increasing (stretched grids need z_wall = 1).  Cell centres are face midpoints (N10). */
+typedef struct {
+    int nx, ny, nz;
+    double lx, ly, lz;
+    const double *zf;
+} fizzy_grid;
+
+/* Boundary conditions: x, y always periodic (all BASELINE.json configs). */
+typedef struct {
+    int z_wall;        /* 0: periodic z; 1: no-slip, impermeable walls at z = 0 and z = lz */
+    double t_wall[2];  /* Dirichlet temperature at the bottom, top wall (heat on) */
+} fizzy_bc;
+
+/* Physical parameters.  Index [0] = fluid 1 (phi = 1), [1] = fluid 2 (phi = 0). */
+typedef struct {
+    double rho[2], mu[2], kth[2], cp[2];
+    double sigma;                 /* surface tension coefficient (CSF: sigma*kappa*grad phi) */
+    double eps;                   /* interface thickness parameter of ACDI */
+    double delta;                 /* regulariser in psi = eps*ln((phi+delta)/(1-phi+delta)); N2: 1e-100 */
+    double gamma_rel, gamma_abs;  /* Gamma = gamma_rel*max|u| + gamma_abs, refreshed at stage 0 (N15) */
+    double g[3];                  /* gravity */
+    double rho_ref;               /* gravity enters as g*(1 - rho_ref/rho_f) (N12) */
+    double beta, t_ref;           /* Oberbeck-Boussinesq: -g*beta*(T - t_ref) (N13) */
+    double force[3];              /* uniform body acceleration */
+    double lin_forcing;           /* Lundgren linear forcing coefficient A: + A*u (N22) */
+    int heat;                     /* 1: evolve the temperature equation */
+} fizzy_props;
+
+/* Bytes of device workspace fizzy_create needs for this grid / property set (0 on bad input). */
+size_t fizzy_workspace_bytes(const fizzy_grid *grid, const fizzy_bc *bc, const fizzy_props *props);
+
+/* Create a context.  `dev_workspace` must hold at least fizzy_workspace_bytes() bytes, be
+ * 256-byte aligned and outlive the context.  `cuda_stream` is a cudaStream_t (NULL = default
+ * stream).  Builds the 1-D metric tables, FFT twiddles, modified wavenumbers
+ * lam_x(l) = -4 sin^2(pi l/nx)/dx^2 (lam_y likewise) and the z-tridiagonal elimination tables.
+ * FIZZY_EINVAL: nx, ny not powers of two in [8,1024], nz < 4, lengths <= 0, non-monotone zf,
+ * zf given with z_wall = 0, rho <= 0, mu < 0, eps <= 0, delta <= 0, cp or kth <= 0 with heat on,
+ * misaligned workspace.  FIZZY_ENOMEM: workspace too small. */
+fizzy_status fizzy_create(const fizzy_grid *grid, const fizzy_bc *bc, const fizzy_props *props,
+                          void *dev_workspace, size_t workspace_bytes, void *cuda_stream,
+                          fizzy_ctx **out);
+
+fizzy_status fizzy_destroy(fizzy_ctx *ctx);
+
+/* Load the prognostic fields (host or device pointers, N doubles each).  NULL = leave unchanged
+ * (the workspace starts zero-filled).  p_prev == NULL sets p_prev := p when p is given.
+ * Zeroes the RK history, enforces w[:,:,nz-1] = 0 with walls, recomputes max|u| and the
+ * interface quantities of phi, and resets the stage counter to 0. */
+fizzy_status fizzy_set_fields(fizzy_ctx *ctx, const double *u, const double *v, const double *w,
+                              const double *p, const double *phi, const double *T,
+                              const double *p_prev);
+
+/* One RK3 substep, stage = 0, 1, 2 in this order (N1: Wray coefficients gamma = 8/15, 5/12,
+ * 3/4; zeta = 0, -17/60, -5/12).  Steps S0-S5 of DESIGN.md: Gamma latch (stage 0), ACDI phi
+ * transport, property map, temperature transport (heat on), momentum predictor, Poisson
+ * right-hand side + FFT(x,y) + tridiagonal(z) solve, velocity correction and pressure rotation.
+ * FIZZY_EINVAL: stage not in {0,1,2} or dt <= 0.  FIZZY_ESTATE: fields not set / wrong stage. */
+fizzy_status fizzy_rk3_substep(fizzy_ctx *ctx, int stage, double dt);
+
+/* Solve Lap p = rhs with the context's grid and z boundary condition (periodic x, y; periodic
+ * or homogeneous Neumann z): FFT in x and y, tridiagonal in z (BASELINE.json:5(iv)).  The
+ * singular mean mode follows N17: last row replaced by p_hat(nz-1) = 0, then the dzf-weighted
+ * mean is removed.  rhs and p are N doubles, host or device; they may alias. */
+fizzy_status fizzy_poisson_solve(fizzy_ctx *ctx, const double *rhs, double *p);
+
+/* Copy fields out (host or device pointers); any pointer may be NULL. */
+fizzy_status fizzy_get_fields(fizzy_ctx *ctx, double *u, double *v, double *w, double *p,
+                              double *phi, double *T, double *p_prev);
+
+/* Current Gamma (synchronises the stream).  NaN if ctx is NULL. */
+double fizzy_gamma(fizzy_ctx *ctx);
+
+/* Number of kernels the library has launched on this context so far (host counter). */
+long long fizzy_launch_count(const fizzy_ctx *ctx);
+
+/* Text of the last error on this context ("" if none); static text if ctx is NULL. */
+const char *fizzy_last_error(const fizzy_ctx *ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* FIZZY_H */

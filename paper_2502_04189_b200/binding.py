@@ -1,0 +1,196 @@
+"""Thin ctypes binding of libfizzy.so (include/fizzy.h): same entry-point names, argument
+marshalling only.  PyTorch is used for device memory (the workspace tensor) and the stream.
+
+Importing this module loads the CUDA library and raises if it is missing: there is no CPU
+fallback and nothing here imports the oracle."""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libfizzy.so")
+
+FIZZY_OK, FIZZY_EINVAL, FIZZY_ENOMEM, FIZZY_ECUDA, FIZZY_ESTATE = range(5)
+_STATUS = {0: "FIZZY_OK", 1: "FIZZY_EINVAL", 2: "FIZZY_ENOMEM", 3: "FIZZY_ECUDA", 4: "FIZZY_ESTATE"}
+
+EXPORTS = ["fizzy_workspace_bytes", "fizzy_create", "fizzy_destroy", "fizzy_set_fields",
+           "fizzy_rk3_substep", "fizzy_poisson_solve", "fizzy_get_fields", "fizzy_gamma",
+           "fizzy_launch_count", "fizzy_last_error"]
+
+
+class FizzyGrid(C.Structure):
+    _fields_ = [("nx", C.c_int), ("ny", C.c_int), ("nz", C.c_int),
+                ("lx", C.c_double), ("ly", C.c_double), ("lz", C.c_double),
+                ("zf", C.POINTER(C.c_double))]
+
+
+class FizzyBC(C.Structure):
+    _fields_ = [("z_wall", C.c_int), ("t_wall", C.c_double * 2)]
+
+
+class FizzyProps(C.Structure):
+    _fields_ = [("rho", C.c_double * 2), ("mu", C.c_double * 2), ("kth", C.c_double * 2),
+                ("cp", C.c_double * 2), ("sigma", C.c_double), ("eps", C.c_double),
+                ("delta", C.c_double), ("gamma_rel", C.c_double), ("gamma_abs", C.c_double),
+                ("g", C.c_double * 3), ("rho_ref", C.c_double), ("beta", C.c_double),
+                ("t_ref", C.c_double), ("force", C.c_double * 3), ("lin_forcing", C.c_double),
+                ("heat", C.c_int)]
+
+
+class FizzyError(RuntimeError):
+    def __init__(self, status, text=""):
+        super().__init__("%s%s" % (_STATUS.get(status, status), (": " + text) if text else ""))
+        self.status = status
+
+
+def load_library(path: str = LIB_PATH) -> C.CDLL:
+    if not os.path.exists(path):
+        raise ImportError("libfizzy.so is missing at %s: run `python -m paper_2502_04189_b200.build` "
+                          "(there is no CPU fallback)" % path)
+    lib = C.CDLL(path)
+    vp, dp = C.c_void_p, C.c_void_p  # field pointers are passed as raw addresses (host or device)
+    lib.fizzy_workspace_bytes.restype = C.c_size_t
+    lib.fizzy_workspace_bytes.argtypes = [C.POINTER(FizzyGrid), C.POINTER(FizzyBC), C.POINTER(FizzyProps)]
+    lib.fizzy_create.restype = C.c_int
+    lib.fizzy_create.argtypes = [C.POINTER(FizzyGrid), C.POINTER(FizzyBC), C.POINTER(FizzyProps),
+                                 vp, C.c_size_t, vp, C.POINTER(vp)]
+    lib.fizzy_destroy.restype = C.c_int
+    lib.fizzy_destroy.argtypes = [vp]
+    lib.fizzy_set_fields.restype = C.c_int
+    lib.fizzy_set_fields.argtypes = [vp] + [dp] * 7
+    lib.fizzy_get_fields.restype = C.c_int
+    lib.fizzy_get_fields.argtypes = [vp] + [dp] * 7
+    lib.fizzy_rk3_substep.restype = C.c_int
+    lib.fizzy_rk3_substep.argtypes = [vp, C.c_int, C.c_double]
+    lib.fizzy_poisson_solve.restype = C.c_int
+    lib.fizzy_poisson_solve.argtypes = [vp, dp, dp]
+    lib.fizzy_gamma.restype = C.c_double
+    lib.fizzy_gamma.argtypes = [vp]
+    lib.fizzy_launch_count.restype = C.c_longlong
+    lib.fizzy_launch_count.argtypes = [vp]
+    lib.fizzy_last_error.restype = C.c_char_p
+    lib.fizzy_last_error.argtypes = [vp]
+    return lib
+
+
+_lib = load_library()
+
+
+def structs_from_cfg(cfg: dict):
+    """cfg: the plain dict of paper_2502_04189_b200.workloads (keys nx..t_top, optional zf)."""
+    g = FizzyGrid(cfg["nx"], cfg["ny"], cfg["nz"], cfg["lx"], cfg["ly"], cfg["lz"], None)
+    keep = None
+    if cfg.get("zf") is not None:
+        keep = np.ascontiguousarray(cfg["zf"], dtype=np.float64)
+        g.zf = keep.ctypes.data_as(C.POINTER(C.c_double))
+    bc = FizzyBC(int(cfg.get("z_wall", 0)), (C.c_double * 2)(cfg.get("t_bot", 0.0), cfg.get("t_top", 0.0)))
+    pr = FizzyProps()
+    pr.rho[:] = [cfg["rho1"], cfg["rho2"]]
+    pr.mu[:] = [cfg["mu1"], cfg["mu2"]]
+    pr.kth[:] = [cfg.get("k1", 1.0), cfg.get("k2", 1.0)]
+    pr.cp[:] = [cfg.get("cp1", 1.0), cfg.get("cp2", 1.0)]
+    pr.sigma, pr.eps, pr.delta = cfg.get("sigma", 0.0), cfg["eps"], cfg.get("delta", 1e-100)
+    pr.gamma_rel, pr.gamma_abs = cfg.get("gamma_rel", 0.0), cfg.get("gamma_abs", 0.0)
+    pr.g[:] = [cfg.get("gx", 0.0), cfg.get("gy", 0.0), cfg.get("gz", 0.0)]
+    pr.rho_ref, pr.beta, pr.t_ref = cfg.get("rho_ref", 0.0), cfg.get("beta", 0.0), cfg.get("t_ref", 0.0)
+    pr.force[:] = [cfg.get("fx", 0.0), cfg.get("fy", 0.0), cfg.get("fz", 0.0)]
+    pr.lin_forcing = cfg.get("a_lin", 0.0)
+    pr.heat = int(cfg.get("heat", 0))
+    return g, bc, pr, keep
+
+
+def _addr(a):
+    """Raw address of a torch tensor (host or device), a numpy array, an int, or None."""
+    if a is None:
+        return None
+    if isinstance(a, int):
+        return a
+    if isinstance(a, np.ndarray):
+        assert a.dtype == np.float64 and a.flags["C_CONTIGUOUS"]
+        return a.ctypes.data
+    assert a.dtype.is_floating_point and a.element_size() == 8 and a.is_contiguous()
+    return a.data_ptr()
+
+
+def fizzy_workspace_bytes(cfg: dict) -> int:
+    g, bc, pr, _keep = structs_from_cfg(cfg)
+    return int(_lib.fizzy_workspace_bytes(C.byref(g), C.byref(bc), C.byref(pr)))
+
+
+class Fizzy:
+    """One solver context on the current CUDA device.  Field arguments are torch tensors
+    (cuda or cpu/pinned) or numpy arrays of shape (nz, ny, nx), float64, contiguous."""
+
+    def __init__(self, cfg: dict, stream=None, device="cuda:0"):
+        import torch  # device memory + stream only
+        if not torch.cuda.is_available():
+            raise FizzyError(FIZZY_ECUDA, "no CUDA device: libfizzy has no CPU fallback")
+        self._torch = torch
+        self.cfg = dict(cfg)
+        self.shape = (cfg["nz"], cfg["ny"], cfg["nx"])
+        self.heat = bool(cfg.get("heat", 0))
+        self.device = torch.device(device)
+        g, bc, pr, keep = structs_from_cfg(cfg)
+        nbytes = int(_lib.fizzy_workspace_bytes(C.byref(g), C.byref(bc), C.byref(pr)))
+        if nbytes == 0:
+            raise FizzyError(FIZZY_EINVAL, "invalid grid / bc / props")
+        self.workspace_bytes = nbytes
+        self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+        base = self.workspace.data_ptr()
+        aligned = (base + 255) & ~255
+        self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+        h = C.c_void_p()
+        st = _lib.fizzy_create(C.byref(g), C.byref(bc), C.byref(pr), aligned, nbytes,
+                               self.stream.cuda_stream, C.byref(h))
+        self._h = h if h.value else None
+        self._check(st)
+
+    def _check(self, st):
+        if st != FIZZY_OK:
+            text = _lib.fizzy_last_error(self._h).decode() if self._h else ""
+            raise FizzyError(st, text)
+
+    def close(self):
+        if getattr(self, "_h", None):
+            _lib.fizzy_destroy(self._h)
+            self._h = None
+
+    __del__ = close
+
+    # ---- the C-ABI calls, same names ----
+    def fizzy_set_fields(self, u=None, v=None, w=None, p=None, phi=None, T=None, p_prev=None):
+        self._check(_lib.fizzy_set_fields(self._h, *[_addr(a) for a in (u, v, w, p, phi, T, p_prev)]))
+
+    def fizzy_get_fields(self, u=None, v=None, w=None, p=None, phi=None, T=None, p_prev=None):
+        self._check(_lib.fizzy_get_fields(self._h, *[_addr(a) for a in (u, v, w, p, phi, T, p_prev)]))
+
+    def fizzy_rk3_substep(self, stage: int, dt: float):
+        self._check(_lib.fizzy_rk3_substep(self._h, int(stage), float(dt)))
+
+    def fizzy_poisson_solve(self, rhs, p):
+        self._check(_lib.fizzy_poisson_solve(self._h, _addr(rhs), _addr(p)))
+
+    def fizzy_gamma(self) -> float:
+        return float(_lib.fizzy_gamma(self._h))
+
+    def fizzy_launch_count(self) -> int:
+        return int(_lib.fizzy_launch_count(self._h))
+
+    # ---- conveniences (marshalling only) ----
+    def step(self, dt: float):
+        for s in range(3):
+            self.fizzy_rk3_substep(s, dt)
+
+    def set_fields_numpy(self, **f):
+        self.fizzy_set_fields(**{k: np.ascontiguousarray(a, dtype=np.float64) for k, a in f.items()})
+        self.stream.synchronize()
+
+    def get_fields_numpy(self) -> dict:
+        names = ["u", "v", "w", "p", "phi", "p_prev"] + (["T"] if self.heat else [])
+        out = {n: np.empty(self.shape) for n in names}
+        self.fizzy_get_fields(**out)
+        self.stream.synchronize()
+        return out

@@ -1,0 +1,458 @@
+// fizzy_api.cu -- host side of libfizzy.so: the C ABI of include/fizzy.h, workspace carving,
+// 1-D table construction and the fixed kernel sequence of one RK3 substep.
+#include "../../include/fizzy.h"
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "fz_common.cuh"
+#include "fz_fft.cuh"
+#include "fz_momentum.cuh"
+#include "fz_stencil.cuh"
+#include "fz_tridiag.cuh"
+
+namespace {
+
+const double RK_GAMMA[3] = {8.0 / 15.0, 5.0 / 12.0, 3.0 / 4.0};   // N1 (Wray)
+const double RK_ZETA[3] = {0.0, -17.0 / 60.0, -5.0 / 12.0};
+
+struct Carver {  // hands out 256-byte aligned pieces of the workspace (or just counts)
+    char *base;
+    size_t off;
+    explicit Carver(void *b) : base(static_cast<char *>(b)), off(0) {}
+    void *take(size_t bytes)
+    {
+        void *p = base ? base + off : nullptr;
+        off += (bytes + 255) & ~size_t(255);
+        return p;
+    }
+    double *dbl(size_t n) { return static_cast<double *>(take(n * sizeof(double))); }
+};
+
+}  // namespace
+
+struct fizzy_ctx {
+    FzP P;
+    cudaStream_t stream;
+    bool varrho, varmu, heat, cyclic;
+    int log2nx, log2ny, Sx, Sy;
+    size_t smem_x, smem_y;
+    long long N, M;
+    // fields
+    double *u, *v, *w, *us, *vs, *ws, *hu, *hv, *hw;
+    double *phi, *phin, *hphi;
+    double *p, *pp, *pn;
+    double *T, *Tn, *hT;
+    double *kappa, *divrn, *psi, *rr, *nhx, *nhy, *nhz, *rnx, *rny, *rnz;
+    double2 *spec;
+    double2 *twx, *twy;
+    double *scal;  // [0] running max|u|, [1] Gamma
+    FzTri tri;
+    int fields_set, next_stage;
+    long long launches;
+    std::string err;
+};
+
+namespace {
+
+bool is_pow2(int n) { return n > 0 && (n & (n - 1)) == 0; }
+int ilog2(int n) { int l = 0; while ((1 << l) < n) ++l; return l; }
+
+bool valid_inputs(const fizzy_grid *g, const fizzy_bc *bc, const fizzy_props *pr)
+{
+    if (!g || !bc || !pr) return false;
+    if (!is_pow2(g->nx) || !is_pow2(g->ny) || g->nx < 8 || g->ny < 8 || g->nx > 1024 || g->ny > 1024) return false;
+    if (g->nz < 4) return false;
+    if (!(g->lx > 0) || !(g->ly > 0) || !(g->lz > 0)) return false;
+    if (bc->z_wall != 0 && bc->z_wall != 1) return false;
+    if (g->zf) {
+        if (!bc->z_wall) return false;
+        if (g->zf[0] != 0.0 || g->zf[g->nz] != g->lz) return false;
+        for (int k = 0; k < g->nz; ++k)
+            if (!(g->zf[k + 1] > g->zf[k])) return false;
+    }
+    if (!(pr->rho[0] > 0) || !(pr->rho[1] > 0) || pr->mu[0] < 0 || pr->mu[1] < 0) return false;
+    if (!(pr->eps > 0) || !(pr->delta > 0)) return false;
+    if (pr->heat && (!(pr->cp[0] > 0) || !(pr->cp[1] > 0) || !(pr->kth[0] > 0) || !(pr->kth[1] > 0))) return false;
+    return true;
+}
+
+// carve (or, with base == NULL, just size) the workspace; fills ctx pointers when c != NULL
+size_t layout(fizzy_ctx *c, void *base, const fizzy_grid *g, const fizzy_bc *bc, const fizzy_props *pr,
+              double **ztab /*5 tables*/, double **acoef /*a, c*/, double **lam /*lamx, lamy*/)
+{
+    Carver cv(base);
+    const size_t N = (size_t)g->nx * g->ny * g->nz;
+    const int nxh = g->nx / 2 + 1;
+    const size_t M = (size_t)nxh * g->ny;
+    const bool varrho = pr->rho[0] != pr->rho[1];
+    const bool cyclic = !bc->z_wall;
+    fizzy_ctx dummy;
+    fizzy_ctx *x = c ? c : &dummy;
+    double **f[] = {&x->u, &x->v, &x->w, &x->us, &x->vs, &x->ws, &x->hu, &x->hv, &x->hw, &x->phi, &x->phin,
+                    &x->hphi, &x->p, &x->pp, &x->pn, &x->kappa, &x->divrn, &x->psi, &x->rr, &x->nhx,
+                    &x->nhy, &x->nhz};
+    for (auto q : f) *q = cv.dbl(N);
+    x->rnx = x->rny = x->rnz = nullptr;
+    if (varrho) { x->rnx = cv.dbl(N); x->rny = cv.dbl(N); x->rnz = cv.dbl(N); }
+    x->T = x->Tn = x->hT = nullptr;
+    if (pr->heat) { x->T = cv.dbl(N); x->Tn = cv.dbl(N); x->hT = cv.dbl(N); }
+    x->spec = static_cast<double2 *>(cv.take(M * g->nz * sizeof(double2)));
+    x->tri.inv = cv.dbl(M * g->nz);
+    x->tri.e = x->tri.f = x->tri.ginv = nullptr;
+    if (cyclic) { x->tri.e = cv.dbl(M * g->nz); x->tri.f = cv.dbl(M * g->nz); x->tri.ginv = cv.dbl(M); }
+    for (int q = 0; q < 5; ++q) { double *t = cv.dbl(g->nz + 2 * FZ_H); if (ztab) ztab[q] = t; }
+    for (int q = 0; q < 2; ++q) { double *t = cv.dbl(g->nz); if (acoef) acoef[q] = t; }
+    { double *t = cv.dbl(nxh); if (lam) lam[0] = t; t = cv.dbl(g->ny); if (lam) lam[1] = t; }
+    x->twx = static_cast<double2 *>(cv.take(g->nx * sizeof(double2)));
+    x->twy = static_cast<double2 *>(cv.take(g->ny * sizeof(double2)));
+    x->scal = cv.dbl(4);
+    return cv.off;
+}
+
+fizzy_status fail(fizzy_ctx *c, fizzy_status s, const char *what)
+{
+    if (c) c->err = what;
+    return s;
+}
+
+fizzy_status cuda_fail(fizzy_ctx *c, cudaError_t e, const char *where)
+{
+    if (c) c->err = std::string(where) + ": " + cudaGetErrorString(e);
+    return FIZZY_ECUDA;
+}
+
+#define FZ_CUDA(call)                                                   \
+    do {                                                                \
+        cudaError_t e_ = (call);                                        \
+        if (e_ != cudaSuccess) return cuda_fail(c, e_, #call);          \
+    } while (0)
+
+#define FZ_LAUNCHED(name)                                               \
+    do {                                                                \
+        ++c->launches;                                                  \
+        cudaError_t e_ = cudaPeekAtLastError();                         \
+        if (e_ != cudaSuccess) return cuda_fail(c, e_, name);           \
+    } while (0)
+
+void cell_launch(const fizzy_ctx *c, dim3 &grid, dim3 &block)
+{
+    const int bx = c->P.nx < 64 ? c->P.nx : 64;
+    int by = 256 / bx;
+    if (by > c->P.ny) by = c->P.ny;
+    block = dim3(bx, by, 1);
+    grid = dim3(c->P.nx / bx, c->P.ny / by, c->P.nz);
+}
+
+}  // namespace
+
+// =====================================================================================
+extern "C" size_t fizzy_workspace_bytes(const fizzy_grid *grid, const fizzy_bc *bc, const fizzy_props *props)
+{
+    if (!valid_inputs(grid, bc, props)) return 0;
+    return layout(nullptr, nullptr, grid, bc, props, nullptr, nullptr, nullptr);
+}
+
+extern "C" fizzy_status fizzy_create(const fizzy_grid *grid, const fizzy_bc *bc, const fizzy_props *props,
+                                     void *dev_workspace, size_t workspace_bytes, void *cuda_stream,
+                                     fizzy_ctx **out)
+{
+    if (!out) return FIZZY_EINVAL;
+    *out = nullptr;
+    if (!valid_inputs(grid, bc, props)) return FIZZY_EINVAL;
+    if (!dev_workspace || (reinterpret_cast<uintptr_t>(dev_workspace) & 255)) return FIZZY_EINVAL;
+    if (workspace_bytes < layout(nullptr, nullptr, grid, bc, props, nullptr, nullptr, nullptr)) return FIZZY_ENOMEM;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) return FIZZY_ECUDA;  // no CPU fallback
+    fizzy_ctx *c = new (std::nothrow) fizzy_ctx();
+    if (!c) return FIZZY_ENOMEM;
+    *out = c;  // returned even on a CUDA failure below so that fizzy_last_error can be read
+    c->stream = static_cast<cudaStream_t>(cuda_stream);
+    c->fields_set = 0;
+    c->next_stage = 0;
+    c->launches = 0;
+
+    const int nx = grid->nx, ny = grid->ny, nz = grid->nz;
+    double *ztab[5], *acoef[2], *lam[2];
+    const size_t used = layout(c, dev_workspace, grid, bc, props, ztab, acoef, lam);
+    FZ_CUDA(cudaMemsetAsync(dev_workspace, 0, used, c->stream));
+
+    FzP &P = c->P;
+    std::memset(&P, 0, sizeof(P));
+    P.nx = nx; P.ny = ny; P.nz = nz; P.nxh = nx / 2 + 1;
+    P.z_wall = bc->z_wall; P.heat = props->heat ? 1 : 0;
+    P.kzf = bc->z_wall ? nz - 1 : nz;
+    P.N = (long long)nx * ny * nz; P.sxy = (long long)nx * ny;
+    P.dx = grid->lx / nx; P.dy = grid->ly / ny; P.idx = 1.0 / P.dx; P.idy = 1.0 / P.dy;
+    P.rho1 = props->rho[0]; P.rho2 = props->rho[1]; P.mu1 = props->mu[0]; P.mu2 = props->mu[1];
+    P.k1 = props->kth[0]; P.k2 = props->kth[1]; P.cp1 = props->cp[0]; P.cp2 = props->cp[1];
+    P.sigma = props->sigma; P.eps = props->eps; P.delta = props->delta;
+    P.gamma_rel = props->gamma_rel; P.gamma_abs = props->gamma_abs;
+    P.gx = props->g[0]; P.gy = props->g[1]; P.gz = props->g[2];
+    P.rho_ref = props->rho_ref; P.beta = props->beta; P.t_ref = props->t_ref;
+    P.fx = props->force[0]; P.fy = props->force[1]; P.fz = props->force[2];
+    P.a_lin = props->lin_forcing;
+    P.t_bot = bc->t_wall[0]; P.t_top = bc->t_wall[1];
+    P.rho0 = std::fmin(P.rho1, P.rho2); P.drho = P.rho1 - P.rho2;
+    c->N = P.N; c->M = (long long)P.nxh * ny;
+    c->varrho = P.rho1 != P.rho2; c->varmu = P.mu1 != P.mu2; c->heat = P.heat != 0; c->cyclic = !bc->z_wall;
+    c->log2nx = ilog2(nx); c->log2ny = ilog2(ny);
+    c->Sx = nx >= 1024 ? 4 : (nx >= 32 ? 8 : 256 / nx);   // 1024-point lines: 512 threads per CTA
+    c->Sy = ny >= 1024 ? 4 : (ny >= 32 ? 8 : 256 / ny);
+    c->smem_x = (size_t)nx * (c->Sx + 1) * sizeof(double2);
+    c->smem_y = (size_t)ny * (c->Sy + 1) * sizeof(double2);
+
+    // ---- 1-D z metrics with ghosts (walls mirror, periodic wraps), N10: centres = face midpoints
+    const int nzt = nz + 2 * FZ_H;
+    std::vector<double> dzf(nzt), dzc(nzt, 0.0), idzf(nzt), idzc(nzt, 0.0), igz(nzt, 0.0);
+    for (int k = 0; k < nz; ++k) dzf[k + FZ_H] = grid->zf ? grid->zf[k + 1] - grid->zf[k] : grid->lz / nz;
+    for (int g = 1; g <= FZ_H; ++g) {
+        dzf[FZ_H - g] = bc->z_wall ? dzf[FZ_H + g - 1] : dzf[FZ_H + nz - g];
+        dzf[FZ_H + nz - 1 + g] = bc->z_wall ? dzf[FZ_H + nz - g] : dzf[FZ_H + g - 1];
+    }
+    for (int q = 0; q < nzt - 1; ++q) dzc[q] = 0.5 * (dzf[q] + dzf[q + 1]);
+    dzc[nzt - 1] = dzc[nzt - 2];
+    for (int q = 0; q < nzt; ++q) { idzf[q] = 1.0 / dzf[q]; idzc[q] = 1.0 / dzc[q]; }
+    for (int q = 1; q < nzt; ++q) igz[q] = 1.0 / (dzc[q] + dzc[q - 1]);
+    const std::vector<double> *tabs[5] = {&dzf, &dzc, &idzf, &idzc, &igz};
+    for (int q = 0; q < 5; ++q)
+        FZ_CUDA(cudaMemcpyAsync(ztab[q], tabs[q]->data(), nzt * sizeof(double), cudaMemcpyHostToDevice, c->stream));
+    P.dzf = ztab[0] + FZ_H; P.dzc = ztab[1] + FZ_H; P.idzf = ztab[2] + FZ_H; P.idzc = ztab[3] + FZ_H;
+    P.igz = ztab[4] + FZ_H;
+
+    // ---- tridiagonal coefficients, modified wavenumbers, twiddles
+    std::vector<double> a(nz), cc(nz), lx(P.nxh), ly(ny);
+    for (int k = 0; k < nz; ++k) {
+        a[k] = 1.0 / (dzf[k + FZ_H] * dzc[k - 1 + FZ_H]);
+        cc[k] = 1.0 / (dzf[k + FZ_H] * dzc[k + FZ_H]);
+    }
+    if (bc->z_wall) { a[0] = 0.0; cc[nz - 1] = 0.0; }
+    for (int l = 0; l < P.nxh; ++l) { const double s = std::sin(M_PI * l / nx); lx[l] = -4.0 * s * s / (P.dx * P.dx); }
+    for (int m = 0; m < ny; ++m) { const double s = std::sin(M_PI * m / ny); ly[m] = -4.0 * s * s / (P.dy * P.dy); }
+    std::vector<double2> twx(nx), twy(ny);
+    for (int q = 0; q < nx; ++q) { const double t = -2.0 * M_PI * q / nx; twx[q] = make_double2(std::cos(t), std::sin(t)); }
+    for (int q = 0; q < ny; ++q) { const double t = -2.0 * M_PI * q / ny; twy[q] = make_double2(std::cos(t), std::sin(t)); }
+    FZ_CUDA(cudaMemcpyAsync(acoef[0], a.data(), nz * sizeof(double), cudaMemcpyHostToDevice, c->stream));
+    FZ_CUDA(cudaMemcpyAsync(acoef[1], cc.data(), nz * sizeof(double), cudaMemcpyHostToDevice, c->stream));
+    FZ_CUDA(cudaMemcpyAsync(lam[0], lx.data(), P.nxh * sizeof(double), cudaMemcpyHostToDevice, c->stream));
+    FZ_CUDA(cudaMemcpyAsync(lam[1], ly.data(), ny * sizeof(double), cudaMemcpyHostToDevice, c->stream));
+    FZ_CUDA(cudaMemcpyAsync(c->twx, twx.data(), nx * sizeof(double2), cudaMemcpyHostToDevice, c->stream));
+    FZ_CUDA(cudaMemcpyAsync(c->twy, twy.data(), ny * sizeof(double2), cudaMemcpyHostToDevice, c->stream));
+    FZ_CUDA(cudaStreamSynchronize(c->stream));  // the host vectors go out of scope below
+
+    c->tri.a = acoef[0]; c->tri.c = acoef[1]; c->tri.lamx = lam[0]; c->tri.lamy = lam[1];
+    c->tri.M = c->M; c->tri.cyclic = c->cyclic ? 1 : 0;
+    k_tri_tables<<<(unsigned)((c->M + 127) / 128), 128, 0, c->stream>>>(P, c->tri);
+    FZ_LAUNCHED("k_tri_tables");
+
+    // dynamic shared memory opt-in for the FFT kernels
+    FZ_CUDA(cudaFuncSetAttribute(k_fftx_fwd<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_x));
+    FZ_CUDA(cudaFuncSetAttribute(k_fftx_fwd<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_x));
+    FZ_CUDA(cudaFuncSetAttribute(k_fftx_inv, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_x));
+    FZ_CUDA(cudaFuncSetAttribute(k_ffty<-1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_y));
+    FZ_CUDA(cudaFuncSetAttribute(k_ffty<+1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_y));
+    return FIZZY_OK;
+}
+
+extern "C" fizzy_status fizzy_destroy(fizzy_ctx *c)
+{
+    if (!c) return FIZZY_EINVAL;
+    cudaStreamSynchronize(c->stream);
+    delete c;
+    return FIZZY_OK;
+}
+
+extern "C" const char *fizzy_last_error(const fizzy_ctx *c) { return c ? c->err.c_str() : "null context"; }
+extern "C" long long fizzy_launch_count(const fizzy_ctx *c) { return c ? c->launches : 0; }
+
+extern "C" double fizzy_gamma(fizzy_ctx *c)
+{
+    if (!c) return NAN;
+    double g = NAN;
+    if (cudaMemcpyAsync(&g, c->scal + 1, sizeof(double), cudaMemcpyDeviceToHost, c->stream) != cudaSuccess) return NAN;
+    if (cudaStreamSynchronize(c->stream) != cudaSuccess) return NAN;
+    return g;
+}
+
+// =====================================================================================
+namespace {
+
+// interface quantities of c->phi -> kappa, divRn (and Rn when rho1 != rho2): kernel group (a)
+fizzy_status run_interface(fizzy_ctx *c)
+{
+    dim3 grid, block;
+    cell_launch(c, grid, block);
+    k_iface_psi<<<grid, block, 0, c->stream>>>(c->P, c->phi, c->psi, c->rr);
+    FZ_LAUNCHED("k_iface_psi");
+    k_iface_nhat<<<grid, block, 0, c->stream>>>(c->P, c->psi, c->nhx, c->nhy, c->nhz);
+    FZ_LAUNCHED("k_iface_nhat");
+    if (c->varrho)
+        k_iface_flux<true><<<grid, block, 0, c->stream>>>(c->P, c->phi, c->rr, c->nhx, c->nhy, c->nhz, c->kappa,
+                                                          c->divrn, c->rnx, c->rny, c->rnz);
+    else
+        k_iface_flux<false><<<grid, block, 0, c->stream>>>(c->P, c->phi, c->rr, c->nhx, c->nhy, c->nhz, c->kappa,
+                                                           c->divrn, nullptr, nullptr, nullptr);
+    FZ_LAUNCHED("k_iface_flux");
+    return FIZZY_OK;
+}
+
+// spectral part of S4 on c->spec (forward x-transform already done): y-FFT, z-solve, gauge, inverse
+fizzy_status run_spectral_solve(fizzy_ctx *c, double *dst)
+{
+    const FzP &P = c->P;
+    const dim3 gy((P.nxh + c->Sy - 1) / c->Sy, P.nz);
+    const int ty = c->Sy * P.ny / 8, tx = c->Sx * P.nx / 8;
+    k_ffty<-1><<<gy, ty, c->smem_y, c->stream>>>(P, c->spec, c->twy, c->log2ny, c->Sy);
+    FZ_LAUNCHED("k_ffty<-1>");
+    const unsigned gt = (unsigned)((c->M + 127) / 128);
+    if (c->cyclic) k_tridiag<true><<<gt, 128, 0, c->stream>>>(P, c->tri, c->spec);
+    else k_tridiag<false><<<gt, 128, 0, c->stream>>>(P, c->tri, c->spec);
+    FZ_LAUNCHED("k_tridiag");
+    k_gauge<<<1, 256, 0, c->stream>>>(P, c->spec, c->M);
+    FZ_LAUNCHED("k_gauge");
+    k_ffty<+1><<<gy, ty, c->smem_y, c->stream>>>(P, c->spec, c->twy, c->log2ny, c->Sy);
+    FZ_LAUNCHED("k_ffty<+1>");
+    const long long nlines = (long long)P.ny * P.nz;
+    const unsigned gx = (unsigned)((nlines + 2 * c->Sx - 1) / (2 * c->Sx));
+    k_fftx_inv<<<gx, tx, c->smem_x, c->stream>>>(P, c->spec, dst, 1.0 / ((double)P.nx * (double)P.ny), c->twx,
+                                                 c->log2nx, c->Sx);
+    FZ_LAUNCHED("k_fftx_inv");
+    return FIZZY_OK;
+}
+
+template <bool VR, bool VM>
+void launch_momentum(fizzy_ctx *c, dim3 grid, dim3 block, const FzMomArgs &A)
+{
+    if (c->heat) k_momentum<VR, VM, true><<<grid, block, 0, c->stream>>>(c->P, A);
+    else k_momentum<VR, VM, false><<<grid, block, 0, c->stream>>>(c->P, A);
+}
+
+}  // namespace
+
+extern "C" fizzy_status fizzy_set_fields(fizzy_ctx *c, const double *u, const double *v, const double *w,
+                                         const double *p, const double *phi, const double *T,
+                                         const double *p_prev)
+{
+    if (!c) return FIZZY_EINVAL;
+    const size_t B = (size_t)c->N * sizeof(double);
+    const double *src[] = {u, v, w, p, phi, c->heat ? T : nullptr};
+    double *dst[] = {c->u, c->v, c->w, c->p, c->phi, c->T};
+    for (int q = 0; q < 6; ++q)
+        if (src[q]) FZ_CUDA(cudaMemcpyAsync(dst[q], src[q], B, cudaMemcpyDefault, c->stream));
+    if (p_prev) FZ_CUDA(cudaMemcpyAsync(c->pp, p_prev, B, cudaMemcpyDefault, c->stream));
+    else if (p) FZ_CUDA(cudaMemcpyAsync(c->pp, c->p, B, cudaMemcpyDeviceToDevice, c->stream));
+    double *hist[] = {c->hphi, c->hu, c->hv, c->hw, c->hT};
+    for (double *h : hist)
+        if (h) FZ_CUDA(cudaMemsetAsync(h, 0, B, c->stream));
+    if (c->P.z_wall) {
+        k_zero_plane<<<(unsigned)((c->P.sxy + 255) / 256), 256, 0, c->stream>>>(c->P, c->w);
+        FZ_LAUNCHED("k_zero_plane");
+    }
+    const double init[2] = {0.0, c->P.gamma_abs};
+    FZ_CUDA(cudaMemcpyAsync(c->scal, init, sizeof(init), cudaMemcpyHostToDevice, c->stream));
+    FZ_CUDA(cudaStreamSynchronize(c->stream));  // `init` is a stack variable
+    k_absmax3<<<148 * 8, 256, 0, c->stream>>>(c->P, c->u, c->v, c->w, c->scal);
+    FZ_LAUNCHED("k_absmax3");
+    fizzy_status s = run_interface(c);
+    if (s != FIZZY_OK) return s;
+    c->fields_set = 1;
+    c->next_stage = 0;
+    return FIZZY_OK;
+}
+
+extern "C" fizzy_status fizzy_get_fields(fizzy_ctx *c, double *u, double *v, double *w, double *p, double *phi,
+                                         double *T, double *p_prev)
+{
+    if (!c) return FIZZY_EINVAL;
+    const size_t B = (size_t)c->N * sizeof(double);
+    double *dst[] = {u, v, w, p, phi, c->heat ? T : nullptr, p_prev};
+    const double *src[] = {c->u, c->v, c->w, c->p, c->phi, c->T, c->pp};
+    for (int q = 0; q < 7; ++q)
+        if (dst[q]) FZ_CUDA(cudaMemcpyAsync(dst[q], src[q], B, cudaMemcpyDefault, c->stream));
+    return FIZZY_OK;
+}
+
+extern "C" fizzy_status fizzy_rk3_substep(fizzy_ctx *c, int stage, double dt)
+{
+    if (!c) return FIZZY_EINVAL;
+    if (stage < 0 || stage > 2 || !(dt > 0.0)) return fail(c, FIZZY_EINVAL, "stage must be 0,1,2 and dt > 0");
+    if (!c->fields_set) return fail(c, FIZZY_ESTATE, "fizzy_set_fields has not been called");
+    if (stage != c->next_stage) return fail(c, FIZZY_ESTATE, "stages must be called in the order 0,1,2");
+    const FzP &P = c->P;
+    const double gs = RK_GAMMA[stage], zs = RK_ZETA[stage], as = gs + zs;
+    dim3 grid, block;
+    cell_launch(c, grid, block);
+    fizzy_status s;
+
+    // S0: latch Gamma = gamma_rel * max|u| + gamma_abs (N15)
+    if (stage == 0) {
+        k_latch_gamma<<<1, 1, 0, c->stream>>>(P, c->scal);
+        FZ_LAUNCHED("k_latch_gamma");
+    }
+    // S1: phi transport (divRn holds D(R/Gamma) of the current phi)
+    k_phi_update<<<grid, block, 0, c->stream>>>(P, c->phi, c->u, c->v, c->w, c->divrn, c->hphi, c->phin, c->scal,
+                                                dt, gs, zs);
+    FZ_LAUNCHED("k_phi_update");
+    std::swap(c->phi, c->phin);
+    // interface quantities of phi_new (N6): used by S3 now and by S1 of the next substep
+    if ((s = run_interface(c)) != FIZZY_OK) return s;
+    // S2b: temperature
+    if (c->heat) {
+        k_temp_update<<<grid, block, 0, c->stream>>>(P, c->T, c->phi, c->u, c->v, c->w, c->hT, c->Tn, dt, gs, zs);
+        FZ_LAUNCHED("k_temp_update");
+        std::swap(c->T, c->Tn);
+    }
+    // S2 + S3: property map on the fly, momentum predictor -> u**
+    FzMomArgs A;
+    A.u = c->u; A.v = c->v; A.w = c->w; A.phi = c->phi; A.kappa = c->kappa;
+    A.rnx = c->rnx; A.rny = c->rny; A.rnz = c->rnz; A.p = c->p; A.pp = c->pp; A.T = c->T;
+    A.us = c->us; A.vs = c->vs; A.ws = c->ws; A.hu = c->hu; A.hv = c->hv; A.hw = c->hw;
+    A.scal = c->scal; A.dt = dt; A.gs = gs; A.zs = zs; A.adt = as * dt;
+    if (c->varrho) { if (c->varmu) launch_momentum<true, true>(c, grid, block, A); else launch_momentum<true, false>(c, grid, block, A); }
+    else { if (c->varmu) launch_momentum<false, true>(c, grid, block, A); else launch_momentum<false, false>(c, grid, block, A); }
+    FZ_LAUNCHED("k_momentum");
+    // S4: b = rho0/(a dt) D(u**), FFT x (fused), FFT y, tridiagonal z, inverse
+    const long long nlines = (long long)P.ny * P.nz;
+    const unsigned gx = (unsigned)((nlines + 2 * c->Sx - 1) / (2 * c->Sx));
+    k_fftx_fwd<true><<<gx, c->Sx * P.nx / 8, c->smem_x, c->stream>>>(P, nullptr, c->us, c->vs, c->ws,
+                                                                     P.rho0 / (as * dt), c->spec, c->twx,
+                                                                     c->log2nx, c->Sx);
+    FZ_LAUNCHED("k_fftx_fwd");
+    if ((s = run_spectral_solve(c, c->pn)) != FIZZY_OK) return s;
+    // S5: correction, pressure rotation
+    if (stage == 2)
+        k_correct<true><<<grid, block, 0, c->stream>>>(P, c->us, c->vs, c->ws, c->pn, c->u, c->v, c->w,
+                                                       as * dt / P.rho0, c->scal);
+    else
+        k_correct<false><<<grid, block, 0, c->stream>>>(P, c->us, c->vs, c->ws, c->pn, c->u, c->v, c->w,
+                                                        as * dt / P.rho0, c->scal);
+    FZ_LAUNCHED("k_correct");
+    double *old_pp = c->pp;
+    c->pp = c->p;
+    c->p = c->pn;
+    c->pn = old_pp;
+    c->next_stage = (stage + 1) % 3;
+    return FIZZY_OK;
+}
+
+extern "C" fizzy_status fizzy_poisson_solve(fizzy_ctx *c, const double *rhs, double *p)
+{
+    if (!c) return FIZZY_EINVAL;
+    if (!rhs || !p) return fail(c, FIZZY_EINVAL, "rhs and p must be non-NULL");
+    const FzP &P = c->P;
+    const size_t B = (size_t)c->N * sizeof(double);
+    FZ_CUDA(cudaMemcpyAsync(c->pn, rhs, B, cudaMemcpyDefault, c->stream));
+    const long long nlines = (long long)P.ny * P.nz;
+    const unsigned gx = (unsigned)((nlines + 2 * c->Sx - 1) / (2 * c->Sx));
+    k_fftx_fwd<false><<<gx, c->Sx * P.nx / 8, c->smem_x, c->stream>>>(P, c->pn, nullptr, nullptr, nullptr, 1.0,
+                                                                      c->spec, c->twx, c->log2nx, c->Sx);
+    FZ_LAUNCHED("k_fftx_fwd<false>");
+    fizzy_status s = run_spectral_solve(c, c->pn);
+    if (s != FIZZY_OK) return s;
+    FZ_CUDA(cudaMemcpyAsync(p, c->pn, B, cudaMemcpyDefault, c->stream));
+    return FIZZY_OK;
+}

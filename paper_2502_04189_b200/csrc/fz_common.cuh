@@ -1,0 +1,64 @@
+// fz_common.cuh -- kernel-side parameter block and small device helpers of libfizzy.
+// Notation follows DESIGN.md "The method" (hc = centre spacing at a face, hf = cell height).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#define FZ_H 2  // ghost entries on each side of the 1-D z metric tables
+
+// Passed by value to every kernel (lives in constant bank 0).
+struct FzP {
+    int nx, ny, nz, nxh;       // nxh = nx/2 + 1 retained x-modes
+    int z_wall, heat;
+    int kzf;                   // z-faces that carry an unknown w: nz (periodic) or nz-1 (walls)
+    long long N;               // nx*ny*nz
+    long long sxy;             // nx*ny (plane stride)
+    double dx, dy, idx, idy;   // spacings and reciprocals
+    // 1-D z metric tables, device pointers already offset by FZ_H (index k = -2 .. nz+1)
+    const double *dzf, *dzc, *idzf, *idzc, *igz;  // igz[k] = 1/(dzc[k] + dzc[k-1])
+    double rho1, rho2, mu1, mu2, k1, k2, cp1, cp2;
+    double sigma, eps, delta, gamma_rel, gamma_abs;
+    double gx, gy, gz, rho_ref, beta, t_ref, fx, fy, fz, a_lin;
+    double t_bot, t_top;
+    double rho0, drho;         // min(rho1, rho2), rho1 - rho2
+};
+
+__device__ __forceinline__ double fz_clip01(double f) { return fmin(fmax(f, 0.0), 1.0); }
+
+// neighbour indices of a cell in the periodic directions
+__device__ __forceinline__ int fz_ip(int i, int n) { return (i + 1 == n) ? 0 : i + 1; }
+__device__ __forceinline__ int fz_im(int i, int n) { return (i == 0) ? n - 1 : i - 1; }
+
+// z neighbours: plane index used for EVEN (mirrored) fields, and flags telling whether the
+// neighbour is a wall ghost.  Periodic z wraps, never a ghost.
+struct FzZ {
+    int km, kp;        // plane indices to read for k-1 / k+1 (mirror at walls, wrap if periodic)
+    bool gm, gp;       // true if k-1 / k+1 lies outside a wall
+};
+__device__ __forceinline__ FzZ fz_zn(const FzP &P, int k)
+{
+    FzZ z;
+    if (P.z_wall) {
+        z.gm = (k == 0);
+        z.gp = (k == P.nz - 1);
+        z.km = z.gm ? 0 : k - 1;
+        z.kp = z.gp ? P.nz - 1 : k + 1;
+    } else {
+        z.gm = z.gp = false;
+        z.km = (k == 0) ? P.nz - 1 : k - 1;
+        z.kp = (k + 1 == P.nz) ? 0 : k + 1;
+    }
+    return z;
+}
+
+// order-preserving max of non-negative doubles through their bit pattern
+__device__ __forceinline__ void fz_atomic_max_nonneg(double *addr, double v)
+{
+    atomicMax(reinterpret_cast<unsigned long long *>(addr),
+              static_cast<unsigned long long>(__double_as_longlong(v)));
+}
+
+__device__ __forceinline__ double2 fz_cmul(double2 a, double2 b)
+{
+    return make_double2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x);
+}

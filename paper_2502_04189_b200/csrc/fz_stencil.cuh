@@ -1,0 +1,212 @@
+// fz_stencil.cuh -- finite-difference kernels of the RK3 substep (DESIGN.md steps S0-S3, S5).
+// One thread per cell, x fastest; 3-D launch: blockIdx.z = k.  Neighbour reuse comes from L1/L2.
+// Passages: BASELINE.json:5 (i)-(iii),(v); readings N2-N15 in DESIGN.md.
+#pragma once
+#include "fz_common.cuh"
+
+#define FZ_CELL_IJK                                          \
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;     \
+    const int j = blockIdx.y * blockDim.y + threadIdx.y;     \
+    const int k = blockIdx.z;                                \
+    if (i >= P.nx || j >= P.ny) return;
+
+// ---------------------------------------------------------------- S0: max |u|, Gamma latch
+__global__ void k_absmax3(FzP P, const double *__restrict__ u, const double *__restrict__ v,
+                          const double *__restrict__ w, double *umax)
+{
+    double m = 0.0;
+    for (long long c = blockIdx.x * (long long)blockDim.x + threadIdx.x; c < P.N;
+         c += (long long)gridDim.x * blockDim.x)
+        m = fmax(m, fmax(fabs(u[c]), fmax(fabs(v[c]), fabs(w[c]))));
+    for (int o = 16; o > 0; o >>= 1) m = fmax(m, __shfl_xor_sync(0xffffffffu, m, o));
+    if ((threadIdx.x & 31) == 0) fz_atomic_max_nonneg(umax, m);
+}
+
+// scal[0] = running max|u| (reset here), scal[1] = Gamma (latched here; N15)
+__global__ void k_latch_gamma(FzP P, double *scal)
+{
+    scal[1] = P.gamma_rel * scal[0] + P.gamma_abs;
+    scal[0] = 0.0;
+}
+
+// ---------------------------------------------------------------- interface quantities (N2-N5)
+// (a) psi = eps ln q, r = sqrt(q), q = (phic+delta)/(1-phic+delta)
+__global__ void k_iface_psi(FzP P, const double *__restrict__ phi, double *__restrict__ psi,
+                            double *__restrict__ rr)
+{
+    FZ_CELL_IJK
+    const long long c = i + (long long)P.nx * (j + (long long)P.ny * k);
+    const double ph = fz_clip01(phi[c]);
+    const double q = (ph + P.delta) / (1.0 - ph + P.delta);
+    psi[c] = P.eps * log(q);
+    rr[c] = sqrt(q);
+}
+
+// (b) nhat = G / max(|G|, 1e-30), G = central difference of psi (mirror at walls)
+__global__ void k_iface_nhat(FzP P, const double *__restrict__ psi, double *__restrict__ nhx,
+                             double *__restrict__ nhy, double *__restrict__ nhz)
+{
+    FZ_CELL_IJK
+    const FzZ z = fz_zn(P, k);
+    const long long row = (long long)P.nx * (j + (long long)P.ny * k);
+    const long long c = row + i;
+    const double gx = (psi[row + fz_ip(i, P.nx)] - psi[row + fz_im(i, P.nx)]) * (0.5 * P.idx);
+    const double gy = (psi[i + (long long)P.nx * (fz_ip(j, P.ny) + (long long)P.ny * k)] -
+                       psi[i + (long long)P.nx * (fz_im(j, P.ny) + (long long)P.ny * k)]) * (0.5 * P.idy);
+    const double gz = (psi[c + (long long)(z.kp - k) * P.sxy] - psi[c + (long long)(z.km - k) * P.sxy]) * P.igz[k];
+    const double mag = sqrt(gx * gx + gy * gy + gz * gz);
+    const double inv = 1.0 / fmax(mag, 1e-30);
+    nhx[c] = gx * inv;
+    nhy[c] = gy * inv;
+    nhz[c] = gz * inv;
+}
+
+// sharpening coefficient 1/4 (1 - tanh^2((psi_a+psi_b)/(4 eps))) = s/(1+s)^2, s = r_a r_b (N3)
+__device__ __forceinline__ double fz_sharp(double ra, double rb)
+{
+    const double s = ra * rb;
+    const double d = 1.0 + s;
+    return s / (d * d);
+}
+
+// (c) Rn = R/Gamma on the three "+" faces, kappa = -D(nf), divRn = D(Rn)
+template <bool STORE_R>
+__global__ void k_iface_flux(FzP P, const double *__restrict__ phi, const double *__restrict__ rr,
+                             const double *__restrict__ nhx, const double *__restrict__ nhy,
+                             const double *__restrict__ nhz, double *__restrict__ kappa,
+                             double *__restrict__ divrn, double *__restrict__ rnx,
+                             double *__restrict__ rny, double *__restrict__ rnz)
+{
+    FZ_CELL_IJK
+    const FzZ z = fz_zn(P, k);
+    const long long pl = (long long)P.ny * k;
+    const long long c = i + P.nx * (j + pl);
+    const long long xp = fz_ip(i, P.nx) + P.nx * (j + pl), xm = fz_im(i, P.nx) + P.nx * (j + pl);
+    const long long yp = i + P.nx * (fz_ip(j, P.ny) + pl), ym = i + P.nx * (fz_im(j, P.ny) + pl);
+    const long long zp = c + (long long)(z.kp - k) * P.sxy, zm = c + (long long)(z.km - k) * P.sxy;
+    const double f0 = phi[c], r0 = rr[c];
+    const double ax = nhx[c], ay = nhy[c], az = nhz[c];
+    // x faces
+    const double nfxp = 0.5 * (ax + nhx[xp]), nfxm = 0.5 * (nhx[xm] + ax);
+    const double Rxp = P.eps * (phi[xp] - f0) * P.idx - fz_sharp(r0, rr[xp]) * nfxp;
+    const double Rxm = P.eps * (f0 - phi[xm]) * P.idx - fz_sharp(rr[xm], r0) * nfxm;
+    // y faces
+    const double nfyp = 0.5 * (ay + nhy[yp]), nfym = 0.5 * (nhy[ym] + ay);
+    const double Ryp = P.eps * (phi[yp] - f0) * P.idy - fz_sharp(r0, rr[yp]) * nfyp;
+    const double Rym = P.eps * (f0 - phi[ym]) * P.idy - fz_sharp(rr[ym], r0) * nfym;
+    // z faces (zero on wall faces)
+    double nfzp = 0.0, nfzm = 0.0, Rzp = 0.0, Rzm = 0.0;
+    if (!z.gp) {
+        nfzp = 0.5 * (az + nhz[zp]);
+        Rzp = P.eps * (phi[zp] - f0) * P.idzc[k] - fz_sharp(r0, rr[zp]) * nfzp;
+    }
+    if (!z.gm) {
+        nfzm = 0.5 * (nhz[zm] + az);
+        Rzm = P.eps * (f0 - phi[zm]) * P.idzc[k - 1] - fz_sharp(rr[zm], r0) * nfzm;
+    }
+    kappa[c] = -((nfxp - nfxm) * P.idx + (nfyp - nfym) * P.idy + (nfzp - nfzm) * P.idzf[k]);
+    divrn[c] = (Rxp - Rxm) * P.idx + (Ryp - Rym) * P.idy + (Rzp - Rzm) * P.idzf[k];
+    if (STORE_R) {
+        rnx[c] = Rxp;
+        rny[c] = Ryp;
+        rnz[c] = Rzp;
+    }
+}
+
+// ---------------------------------------------------------------- S1: ACDI phi transport
+// RHSphi = D(-u_a phibar_a) + Gamma D(Rn);  phi <- phi + dt (g RHS + z RHS_old)   (BASELINE.json:5(i))
+__global__ void k_phi_update(FzP P, const double *__restrict__ phi, const double *__restrict__ u,
+                             const double *__restrict__ v, const double *__restrict__ w,
+                             const double *__restrict__ divrn, double *__restrict__ hphi,
+                             double *__restrict__ phin, const double *__restrict__ scal, double dt,
+                             double gs, double zs)
+{
+    FZ_CELL_IJK
+    const FzZ z = fz_zn(P, k);
+    const long long pl = (long long)P.ny * k;
+    const long long c = i + P.nx * (j + pl);
+    const long long xp = fz_ip(i, P.nx) + P.nx * (j + pl), xm = fz_im(i, P.nx) + P.nx * (j + pl);
+    const long long yp = i + P.nx * (fz_ip(j, P.ny) + pl), ym = i + P.nx * (fz_im(j, P.ny) + pl);
+    const long long zp = c + (long long)(z.kp - k) * P.sxy, zm = c + (long long)(z.km - k) * P.sxy;
+    const double f0 = phi[c];
+    const double Fxp = -u[c] * 0.5 * (f0 + phi[xp]), Fxm = -u[xm] * 0.5 * (phi[xm] + f0);
+    const double Fyp = -v[c] * 0.5 * (f0 + phi[yp]), Fym = -v[ym] * 0.5 * (phi[ym] + f0);
+    const double Fzp = z.gp ? 0.0 : -w[c] * 0.5 * (f0 + phi[zp]);
+    const double Fzm = z.gm ? 0.0 : -w[zm] * 0.5 * (phi[zm] + f0);
+    const double rhs = (Fxp - Fxm) * P.idx + (Fyp - Fym) * P.idy + (Fzp - Fzm) * P.idzf[k] + scal[1] * divrn[c];
+    phin[c] = f0 + dt * (gs * rhs + zs * hphi[c]);
+    hphi[c] = rhs;
+}
+
+// ---------------------------------------------------------------- S2b: temperature transport (N14)
+__global__ void k_temp_update(FzP P, const double *__restrict__ T, const double *__restrict__ phi,
+                              const double *__restrict__ u, const double *__restrict__ v,
+                              const double *__restrict__ w, double *__restrict__ hT,
+                              double *__restrict__ Tn, double dt, double gs, double zs)
+{
+    FZ_CELL_IJK
+    const FzZ z = fz_zn(P, k);
+    const long long pl = (long long)P.ny * k;
+    const long long c = i + P.nx * (j + pl);
+    const long long xp = fz_ip(i, P.nx) + P.nx * (j + pl), xm = fz_im(i, P.nx) + P.nx * (j + pl);
+    const long long yp = i + P.nx * (fz_ip(j, P.ny) + pl), ym = i + P.nx * (fz_im(j, P.ny) + pl);
+    const long long zp = c + (long long)(z.kp - k) * P.sxy, zm = c + (long long)(z.km - k) * P.sxy;
+    const double dk = P.k1 - P.k2;
+    const double t0 = T[c];
+    const double txp = T[xp], txm = T[xm], typ = T[yp], tym = T[ym];
+    const double tzp = z.gp ? 2.0 * P.t_top - t0 : T[zp];
+    const double tzm = z.gm ? 2.0 * P.t_bot - t0 : T[zm];
+    const double phc = fz_clip01(phi[c]);
+    const double k0 = P.k2 + dk * phc;
+    const double kxp = P.k2 + dk * fz_clip01(phi[xp]), kxm = P.k2 + dk * fz_clip01(phi[xm]);
+    const double kyp = P.k2 + dk * fz_clip01(phi[yp]), kym = P.k2 + dk * fz_clip01(phi[ym]);
+    const double kzp = P.k2 + dk * fz_clip01(phi[zp]), kzm = P.k2 + dk * fz_clip01(phi[zm]);
+    const double Axp = -u[c] * 0.5 * (t0 + txp), Axm = -u[xm] * 0.5 * (txm + t0);
+    const double Ayp = -v[c] * 0.5 * (t0 + typ), Aym = -v[ym] * 0.5 * (tym + t0);
+    const double Azp = z.gp ? 0.0 : -w[c] * 0.5 * (t0 + tzp);
+    const double Azm = z.gm ? 0.0 : -w[zm] * 0.5 * (tzm + t0);
+    const double adv = (Axp - Axm) * P.idx + (Ayp - Aym) * P.idy + (Azp - Azm) * P.idzf[k];
+    const double qxp = 0.5 * (k0 + kxp) * (txp - t0) * P.idx, qxm = 0.5 * (kxm + k0) * (t0 - txm) * P.idx;
+    const double qyp = 0.5 * (k0 + kyp) * (typ - t0) * P.idy, qym = 0.5 * (kym + k0) * (t0 - tym) * P.idy;
+    const double qzp = 0.5 * (k0 + kzp) * (tzp - t0) * P.idzc[k];
+    const double qzm = 0.5 * (kzm + k0) * (t0 - tzm) * P.idzc[k - 1];
+    const double dif = (qxp - qxm) * P.idx + (qyp - qym) * P.idy + (qzp - qzm) * P.idzf[k];
+    const double rho = P.rho2 + P.drho * phc, cp = P.cp2 + (P.cp1 - P.cp2) * phc;
+    const double rhs = adv + dif / (rho * cp);
+    Tn[c] = t0 + dt * (gs * rhs + zs * hT[c]);
+    hT[c] = rhs;
+}
+
+// ---------------------------------------------------------------- S5: velocity correction
+// u = u** - (a dt / rho0) d_a p_new  (the p_hat part of BASELINE.json:5(v) is already in u**)
+template <bool WITH_MAX>
+__global__ void k_correct(FzP P, const double *__restrict__ us, const double *__restrict__ vs,
+                          const double *__restrict__ ws, const double *__restrict__ pn,
+                          double *__restrict__ u, double *__restrict__ v, double *__restrict__ w,
+                          double coef /* a dt / rho0 */, double *umax)
+{
+    FZ_CELL_IJK
+    const FzZ z = fz_zn(P, k);
+    const long long pl = (long long)P.ny * k;
+    const long long c = i + P.nx * (j + pl);
+    const double p0 = pn[c];
+    const double un = us[c] - coef * (pn[fz_ip(i, P.nx) + P.nx * (j + pl)] - p0) * P.idx;
+    const double vn = vs[c] - coef * (pn[i + P.nx * (fz_ip(j, P.ny) + pl)] - p0) * P.idy;
+    double wn = 0.0;
+    if (k < P.kzf) wn = ws[c] - coef * (pn[c + (long long)(z.kp - k) * P.sxy] - p0) * P.idzc[k];
+    u[c] = un;
+    v[c] = vn;
+    w[c] = wn;
+    if (WITH_MAX) {
+        double m = fmax(fabs(un), fmax(fabs(vn), fabs(wn)));
+        for (int o = 16; o > 0; o >>= 1) m = fmax(m, __shfl_xor_sync(0xffffffffu, m, o));
+        if (((threadIdx.x + blockDim.x * threadIdx.y) & 31) == 0) fz_atomic_max_nonneg(umax, m);
+    }
+}
+
+// zero the top-wall w plane (w[:,:,nz-1] == 0 with walls)
+__global__ void k_zero_plane(FzP P, double *w)
+{
+    const long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (t < P.sxy) w[(long long)(P.nz - 1) * P.sxy + t] = 0.0;
+}

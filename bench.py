@@ -1,0 +1,312 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the RK3 step of libfizzy.so on B200 (BASELINE.json `metric`:
+fp64 Mcell-substeps/s per RK3 step on 1 B200; achieved HBM GB/s vs peak).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload 3] [--impl fizzy|reference]
+
+A "step" is one full RK3 step = three fizzy_rk3_substep calls (all rows of SURVEY.md 8(a)).
+Workload at N=1: BASELINE.json configs[3], droplet-laden HIT at 512^3 (the size the north-star
+target is quoted on), synthetic seeded inputs from paper_2502_04189_b200.workloads.
+N>1: replicas only: every rank runs the same workload on its own GPU,
+no data-path collective; value = cells*substeps of all ranks / max-over-ranks time.
+
+One JSON line on stdout (rank 0).  `--impl reference` times the CPU oracle on a bounded sample.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from paper_2502_04189_b200 import workloads as W  # noqa: E402
+
+METRIC = "fp64 Mcell-substeps/s per RK3 step"
+UNIT = "Mcell-substeps/s"
+
+# Algorithmic HBM bytes per cell per launch:
+# every N-array a pass must read or write, once; halos and 1-D tables free.
+def algorithmic_bytes_per_cell(cfg):
+    nx = cfg["nx"]
+    spec = 16.0 * (nx // 2 + 1) / nx          # one complex half-spectrum pass, per real cell
+    varrho = cfg["rho1"] != cfg["rho2"]
+    heat = bool(cfg["heat"])
+    b = {
+        "k_phi_update": 64.0,                                   # r phi,u,v,w,hphi,divRn  w phi,hphi
+        "k_iface_psi": 24.0, "k_iface_nhat": 32.0,              # interface kernels (group a)
+        "k_iface_flux": 56.0 + (24.0 if varrho else 0.0),
+        "k_momentum": 112.0 + (40.0 if varrho else 0.0) + (8.0 if heat else 0.0),
+        "k_fftx_fwd": 24.0 + spec, "k_ffty_fwd": 2 * spec, "k_tridiag": 2 * spec,
+        "k_ffty_inv": 2 * spec, "k_fftx_inv": spec + 8.0, "k_correct": 56.0,
+    }
+    if heat:
+        b["k_temp_update"] = 64.0
+    return b
+
+
+def substep_model_bytes(cfg):
+    """328 B per cell per substep with heat off, 400 B with heat on."""
+    return 400.0 if cfg["heat"] else 328.0
+
+
+def measured_peak_gbs():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler(threading.Thread):
+    """nvidia-smi clocks / throttle reasons sampled DURING the timed region."""
+
+    QUERY = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+             "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.index = index
+        self.stop = threading.Event()
+        self.samples = []
+
+    def run(self):
+        while not self.stop.is_set():
+            try:
+                out = subprocess.run(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.QUERY,
+                                      "--format=csv,noheader,nounits"], capture_output=True, text=True, timeout=5).stdout
+                parts = [p.strip() for p in out.strip().split(",")]
+                if len(parts) >= 6:
+                    self.samples.append(parts)
+            except Exception:
+                pass
+            self.stop.wait(0.2)
+
+    def summary(self):
+        if not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["unavailable"]}
+        sm = sorted(float(s[0]) for s in self.samples)
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = [n for q, n in enumerate(names) if any(s[2 + q].lower().startswith("active") for s in self.samples)]
+        return {"sm_mhz": sm[len(sm) // 2], "sm_max_mhz": float(self.samples[0][1]), "reasons": reasons,
+                "samples": len(sm)}
+
+
+def run_reference(args, rank):
+    """The CPU oracle as it stands, on the host cores, on a bounded sample of the workload."""
+    if rank != 0:
+        return
+    import oracle
+    oracle.build()
+    n = args.ref_grid
+    cfg, f, dt, _ = W.make(args.workload, grid=(n, n, n), ndrops=max(1, 200 // (512 // n) ** 3))
+    o = oracle.Oracle(cfg)
+    o.set_fields(**f)
+    for _ in range(args.warmup):
+        o.step(dt)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        o.step(dt)
+    el = time.perf_counter() - t0
+    cells = n ** 3
+    value = cells * 3 * args.steps / el / 1e6
+    sample = "config %d recipe at %d^3, %d RK3 steps" % (args.workload, n, args.steps)
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * el / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": W.NAMES[args.workload], "sample": sample},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
+                             "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def cpu_baseline(args):
+    """Oracle timed on a bounded sample (one RK3 step of the same recipe at --cpu-grid^3)."""
+    import oracle
+    oracle.build()
+    n = args.cpu_grid
+    cfg, f, dt, _ = W.make(args.workload, grid=(n, n, n), ndrops=max(1, 200 // (512 // n) ** 3))
+    o = oracle.Oracle(cfg)
+    o.set_fields(**f)
+    t0 = time.perf_counter()
+    o.step(dt)
+    el = time.perf_counter() - t0
+    o.close()
+    return {"value": n ** 3 * 3 / el / 1e6, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
+            "sample": "config %d recipe at %d^3, 1 RK3 step, %.1f s" % (args.workload, n, el)}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--workload", type=int, default=3, help="BASELINE.json config index (0-based)")
+    ap.add_argument("--grid", type=int, nargs=3, default=None, help="override nx ny nz (debug)")
+    ap.add_argument("--impl", default="fizzy", choices=["fizzy", "reference"])
+    ap.add_argument("--cpu-grid", type=int, default=256)
+    ap.add_argument("--ref-grid", type=int, default=128)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "fizzy" else args.warmup
+
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+
+    if args.impl == "reference":
+        run_reference(args, rank)
+        return
+
+    import torch
+    from paper_2502_04189_b200.binding import Fizzy  # raises if libfizzy.so is missing
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (libfizzy has no CPU fallback)")
+    torch.cuda.set_device(local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+
+    cfg, f, dt, _ = W.make(args.workload, grid=tuple(args.grid) if args.grid else None)
+    cells = cfg["nx"] * cfg["ny"] * cfg["nz"]
+    fz = Fizzy(cfg, device="cuda:%d" % local_rank)
+    names = ["u", "v", "w", "p", "phi"] + (["T"] if cfg["heat"] else [])
+    dev = {k: torch.from_numpy(f[k]).to("cuda:%d" % local_rank) for k in names}
+    fz.fizzy_set_fields(**dev)
+    torch.cuda.synchronize()
+
+    def barrier():
+        torch.cuda.synchronize()
+        if dist is not None:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    # ---------------- device-resident throughput (value) ----------------
+    for _ in range(args.warmup):
+        fz.step(dt)
+    fz.fizzy_timing_enable(True)
+    fz.fizzy_timing_get(reset=True)
+    barrier()
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    n0 = fz.fizzy_launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(fz.stream)
+    for _ in range(args.steps):
+        fz.step(dt)
+    e1.record(fz.stream)
+    barrier()
+    sampler.stop.set()
+    sampler.join()
+    ms = e0.elapsed_time(e1)
+    launches = fz.fizzy_launch_count() - n0
+    per_kernel = fz.fizzy_timing_get(reset=True)
+    fz.fizzy_timing_enable(False)
+    chk = torch.empty_like(dev["phi"])
+    fz.fizzy_get_fields(phi=chk)
+    torch.cuda.synchronize()
+    finite = bool(torch.isfinite(chk).all().item())
+    if dist is not None:
+        t = torch.tensor([ms], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    value = world * cells * 3 * args.steps / (ms * 1e-3) / 1e6
+
+    # ---------------- roofline of the dominant kernel + per-kernel table ----------------
+    peak, peak_src = measured_peak_gbs()
+    bpc = algorithmic_bytes_per_cell(cfg)
+    table = []
+    for name, (tot_ms, n) in per_kernel.items():
+        if name in bpc and n:
+            avg = tot_ms / n
+            gbs = bpc[name] * cells / (avg * 1e-3) / 1e9
+            table.append({"kernel": name, "ms_per_launch": round(avg, 4), "launches": n,
+                          "share": tot_ms, "algorithmic_B_per_cell": round(bpc[name], 2),
+                          "achieved_GBs": round(gbs, 1), "frac": round(gbs / peak, 4)})
+    tot = sum(r["share"] for r in table) or 1.0
+    for r in table:
+        r["share"] = round(r["share"] / tot, 4)
+    table.sort(key=lambda r: -r["share"])
+    top = table[0] if table else None
+    sub_ms = ms / (3 * args.steps)
+    sub_gbs = substep_model_bytes(cfg) * cells / (sub_ms * 1e-3) / 1e9
+    roofline = None
+    if top:
+        roofline = {"bound": "hbm", "kernel": top["kernel"], "achieved": top["achieved_GBs"], "peak": peak,
+                    "unit": "GB/s", "frac": top["frac"], "traffic": None, "peak_source": peak_src}
+    # ncu DRAM traffic per launch of the dominant kernel, if a summary has been committed
+    try:
+        with open(os.path.join(ROOT, "profiles", "traffic.json")) as fh:
+            tr = json.load(fh)
+        if roofline and tr.get("workload") == cfg["name"] and roofline["kernel"] in tr.get("bytes_per_launch", {}):
+            roofline["traffic"] = tr["bytes_per_launch"][roofline["kernel"]]
+    except Exception:
+        pass
+
+    # ---------------- end to end through the C ABI with HOST buffers ----------------
+    e2e = None
+    if not args.no_e2e:
+        hin = {k: torch.from_numpy(f[k]).pin_memory() for k in names}
+        hout = {k: torch.empty_like(hin[k]).pin_memory() for k in names}
+        nb = cells * 8
+        ke = max(1, min(args.steps, 3))
+        fz.fizzy_set_fields(**hin)
+        fz.step(dt)
+        fz.fizzy_get_fields(**hout)
+        barrier()
+        e0.record(fz.stream)
+        for _ in range(ke):
+            fz.fizzy_set_fields(**hin)      # H2D of the step's inputs (pinned host memory)
+            fz.step(dt)
+            fz.fizzy_get_fields(**hout)     # D2H of the step's result
+        e1.record(fz.stream)
+        barrier()
+        ems = e0.elapsed_time(e1)
+        if dist is not None:
+            t = torch.tensor([ems], device="cuda", dtype=torch.float64)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            ems = float(t.item())
+        e2e = {"value": world * cells * 3 * ke / (ems * 1e-3) / 1e6, "unit": UNIT,
+               "h2d_bytes_per_step": nb * len(names), "d2h_bytes_per_step": nb * len(names), "steps": ke,
+               "note": "fizzy_set_fields(host) + 3 x fizzy_rk3_substep + fizzy_get_fields(host) per step"}
+
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+    cpu = None
+    if world == 1 and not args.no_cpu_baseline:
+        fz.close()
+        del dev
+        cpu = cpu_baseline(args)
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": cfg["name"], "grid": [cfg["nx"], cfg["ny"], cfg["nz"]], "dt": dt,
+                       "cache": "inputs larger than L2 (each field %.0f MB, 126 MB L2)" % (cells * 8 / 1e6),
+                       "parallelism": "replicas x%d" % world, "finite": finite},
+            "clocks": sampler.summary(), "e2e": e2e, "gpu_launches": launches,
+            "roofline": roofline,
+            "roofline_substep": {"bound": "hbm", "model_B_per_cell": substep_model_bytes(cfg),
+                                 "ms_per_substep": sub_ms, "achieved": round(sub_gbs, 1), "peak": peak,
+                                 "unit": "GB/s", "frac": round(sub_gbs / peak, 4)},
+            "kernels": table, "cpu_baseline": cpu}
+    print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

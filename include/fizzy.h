@@ -125,6 +125,15 @@ double fizzy_gamma(fizzy_ctx *ctx);
 /* Number of kernels the library has launched on this context so far (host counter). */
 long long fizzy_launch_count(const fizzy_ctx *ctx);
 
+/* Measurement aid (used by bench.py for the roofline object): with timing on, every kernel
+ * launch is bracketed by CUDA events recorded on the context's stream.  fizzy_timing_get
+ * synchronises the stream, folds the pending events into per-kernel totals and returns the
+ * name, accumulated milliseconds and launch count of kernel slot `index` (0-based;
+ * FIZZY_EINVAL past the last slot); reset != 0 clears that slot afterwards. */
+fizzy_status fizzy_timing_enable(fizzy_ctx *ctx, int on);
+fizzy_status fizzy_timing_get(fizzy_ctx *ctx, int index, const char **name, double *total_ms,
+                              long long *launches, int reset);
+
 /* Text of the last error on this context ("" if none); static text if ctx is NULL. */
 const char *fizzy_last_error(const fizzy_ctx *ctx);
 

@@ -18,7 +18,7 @@ _STATUS = {0: "FIZZY_OK", 1: "FIZZY_EINVAL", 2: "FIZZY_ENOMEM", 3: "FIZZY_ECUDA"
 
 EXPORTS = ["fizzy_workspace_bytes", "fizzy_create", "fizzy_destroy", "fizzy_set_fields",
            "fizzy_rk3_substep", "fizzy_poisson_solve", "fizzy_get_fields", "fizzy_gamma",
-           "fizzy_launch_count", "fizzy_last_error"]
+           "fizzy_launch_count", "fizzy_last_error", "fizzy_timing_enable", "fizzy_timing_get"]
 
 
 class FizzyGrid(C.Structure):
@@ -71,6 +71,11 @@ def load_library(path: str = LIB_PATH) -> C.CDLL:
     lib.fizzy_gamma.argtypes = [vp]
     lib.fizzy_launch_count.restype = C.c_longlong
     lib.fizzy_launch_count.argtypes = [vp]
+    lib.fizzy_timing_enable.restype = C.c_int
+    lib.fizzy_timing_enable.argtypes = [vp, C.c_int]
+    lib.fizzy_timing_get.restype = C.c_int
+    lib.fizzy_timing_get.argtypes = [vp, C.c_int, C.POINTER(C.c_char_p), C.POINTER(C.c_double),
+                                     C.POINTER(C.c_longlong), C.c_int]
     lib.fizzy_last_error.restype = C.c_char_p
     lib.fizzy_last_error.argtypes = [vp]
     return lib
@@ -178,6 +183,21 @@ class Fizzy:
 
     def fizzy_launch_count(self) -> int:
         return int(_lib.fizzy_launch_count(self._h))
+
+    def fizzy_timing_enable(self, on: bool):
+        self._check(_lib.fizzy_timing_enable(self._h, int(bool(on))))
+
+    def fizzy_timing_get(self, reset: bool = False) -> dict:
+        """{kernel name: (total ms, launches)} for every kernel slot with at least one launch."""
+        out, i = {}, 0
+        while True:
+            name, ms, n = C.c_char_p(), C.c_double(), C.c_longlong()
+            if _lib.fizzy_timing_get(self._h, i, C.byref(name), C.byref(ms), C.byref(n), int(reset)) != FIZZY_OK:
+                break
+            if n.value:
+                out[name.value.decode()] = (ms.value, n.value)
+            i += 1
+        return out
 
     # ---- conveniences (marshalling only) ----
     def step(self, dt: float):

@@ -35,8 +35,22 @@ struct Carver {  // hands out 256-byte aligned pieces of the workspace (or just 
 
 }  // namespace
 
+enum FzKernelId { FZK_LATCH, FZK_PHI, FZK_IPSI, FZK_INHAT, FZK_IFLUX, FZK_TEMP, FZK_MOM, FZK_FFTX_FWD,
+                  FZK_FFTY_FWD, FZK_TRI, FZK_GAUGE, FZK_FFTY_INV, FZK_FFTX_INV, FZK_CORRECT, FZK_OTHER, FZK_COUNT };
+static const char *const FZK_NAME[FZK_COUNT] = {
+    "k_latch_gamma", "k_phi_update", "k_iface_psi", "k_iface_nhat", "k_iface_flux", "k_temp_update", "k_momentum",
+    "k_fftx_fwd", "k_ffty_fwd", "k_tridiag", "k_gauge", "k_ffty_inv", "k_fftx_inv", "k_correct", "other"};
+
+struct FzTimed { int id; cudaEvent_t e0, e1; };
+
 struct fizzy_ctx {
     FzP P;
+    // optional per-kernel timing (fizzy_timing_enable): CUDA events around every launch
+    bool timing = false;
+    std::vector<FzTimed> pending;
+    std::vector<cudaEvent_t> pool;
+    double t_ms[FZK_COUNT] = {0};
+    long long t_n[FZK_COUNT] = {0};
     cudaStream_t stream;
     bool varrho, varmu, heat, cyclic;
     int log2nx, log2ny, Sx, Sy;
@@ -132,11 +146,31 @@ fizzy_status cuda_fail(fizzy_ctx *c, cudaError_t e, const char *where)
         if (e_ != cudaSuccess) return cuda_fail(c, e_, #call);          \
     } while (0)
 
-#define FZ_LAUNCHED(name)                                               \
+cudaEvent_t take_event(fizzy_ctx *c)
+{
+    if (!c->pool.empty()) { cudaEvent_t e = c->pool.back(); c->pool.pop_back(); return e; }
+    cudaEvent_t e = nullptr;
+    cudaEventCreate(&e);
+    return e;
+}
+
+// FZ_TB(id) before a launch, FZ_LAUNCHED(id) after it: counts the launch, checks for a launch
+// error and, in timing mode, brackets the kernel with events on the context's stream.
+#define FZ_TB(id_)                                                      \
+    do {                                                                \
+        if (c->timing) {                                                \
+            FzTimed t_; t_.id = (id_); t_.e0 = take_event(c); t_.e1 = take_event(c); \
+            cudaEventRecord(t_.e0, c->stream);                          \
+            c->pending.push_back(t_);                                   \
+        }                                                               \
+    } while (0)
+
+#define FZ_LAUNCHED(id_)                                                \
     do {                                                                \
         ++c->launches;                                                  \
+        if (c->timing) cudaEventRecord(c->pending.back().e1, c->stream); \
         cudaError_t e_ = cudaPeekAtLastError();                         \
-        if (e_ != cudaSuccess) return cuda_fail(c, e_, name);           \
+        if (e_ != cudaSuccess) return cuda_fail(c, e_, FZK_NAME[id_]);  \
     } while (0)
 
 void cell_launch(const fizzy_ctx *c, dim3 &grid, dim3 &block)
@@ -246,8 +280,9 @@ extern "C" fizzy_status fizzy_create(const fizzy_grid *grid, const fizzy_bc *bc,
 
     c->tri.a = acoef[0]; c->tri.c = acoef[1]; c->tri.lamx = lam[0]; c->tri.lamy = lam[1];
     c->tri.M = c->M; c->tri.cyclic = c->cyclic ? 1 : 0;
+    FZ_TB(FZK_OTHER);
     k_tri_tables<<<(unsigned)((c->M + 127) / 128), 128, 0, c->stream>>>(P, c->tri);
-    FZ_LAUNCHED("k_tri_tables");
+    FZ_LAUNCHED(FZK_OTHER);
 
     // dynamic shared memory opt-in for the FFT kernels
     FZ_CUDA(cudaFuncSetAttribute(k_fftx_fwd<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_x));
@@ -262,7 +297,37 @@ extern "C" fizzy_status fizzy_destroy(fizzy_ctx *c)
 {
     if (!c) return FIZZY_EINVAL;
     cudaStreamSynchronize(c->stream);
+    for (FzTimed &t : c->pending) { cudaEventDestroy(t.e0); cudaEventDestroy(t.e1); }
+    for (cudaEvent_t e : c->pool) cudaEventDestroy(e);
     delete c;
+    return FIZZY_OK;
+}
+
+extern "C" fizzy_status fizzy_timing_enable(fizzy_ctx *c, int on)
+{
+    if (!c) return FIZZY_EINVAL;
+    c->timing = on != 0;
+    return FIZZY_OK;
+}
+
+extern "C" fizzy_status fizzy_timing_get(fizzy_ctx *c, int index, const char **name, double *total_ms,
+                                         long long *launches, int reset)
+{
+    if (!c || index < 0 || index >= FZK_COUNT) return FIZZY_EINVAL;
+    if (!c->pending.empty()) {
+        FZ_CUDA(cudaStreamSynchronize(c->stream));
+        for (FzTimed &t : c->pending) {
+            float ms = 0.f;
+            if (cudaEventElapsedTime(&ms, t.e0, t.e1) == cudaSuccess) { c->t_ms[t.id] += ms; ++c->t_n[t.id]; }
+            c->pool.push_back(t.e0);
+            c->pool.push_back(t.e1);
+        }
+        c->pending.clear();
+    }
+    if (name) *name = FZK_NAME[index];
+    if (total_ms) *total_ms = c->t_ms[index];
+    if (launches) *launches = c->t_n[index];
+    if (reset) { c->t_ms[index] = 0.0; c->t_n[index] = 0; }
     return FIZZY_OK;
 }
 
@@ -286,17 +351,20 @@ fizzy_status run_interface(fizzy_ctx *c)
 {
     dim3 grid, block;
     cell_launch(c, grid, block);
+    FZ_TB(FZK_IPSI);
     k_iface_psi<<<grid, block, 0, c->stream>>>(c->P, c->phi, c->psi, c->rr);
-    FZ_LAUNCHED("k_iface_psi");
+    FZ_LAUNCHED(FZK_IPSI);
+    FZ_TB(FZK_INHAT);
     k_iface_nhat<<<grid, block, 0, c->stream>>>(c->P, c->psi, c->nhx, c->nhy, c->nhz);
-    FZ_LAUNCHED("k_iface_nhat");
+    FZ_LAUNCHED(FZK_INHAT);
+    FZ_TB(FZK_IFLUX);
     if (c->varrho)
         k_iface_flux<true><<<grid, block, 0, c->stream>>>(c->P, c->phi, c->rr, c->nhx, c->nhy, c->nhz, c->kappa,
                                                           c->divrn, c->rnx, c->rny, c->rnz);
     else
         k_iface_flux<false><<<grid, block, 0, c->stream>>>(c->P, c->phi, c->rr, c->nhx, c->nhy, c->nhz, c->kappa,
                                                            c->divrn, nullptr, nullptr, nullptr);
-    FZ_LAUNCHED("k_iface_flux");
+    FZ_LAUNCHED(FZK_IFLUX);
     return FIZZY_OK;
 }
 
@@ -306,21 +374,26 @@ fizzy_status run_spectral_solve(fizzy_ctx *c, double *dst)
     const FzP &P = c->P;
     const dim3 gy((P.nxh + c->Sy - 1) / c->Sy, P.nz);
     const int ty = c->Sy * P.ny / 8, tx = c->Sx * P.nx / 8;
+    FZ_TB(FZK_FFTY_FWD);
     k_ffty<-1><<<gy, ty, c->smem_y, c->stream>>>(P, c->spec, c->twy, c->log2ny, c->Sy);
-    FZ_LAUNCHED("k_ffty<-1>");
+    FZ_LAUNCHED(FZK_FFTY_FWD);
     const unsigned gt = (unsigned)((c->M + 127) / 128);
+    FZ_TB(FZK_TRI);
     if (c->cyclic) k_tridiag<true><<<gt, 128, 0, c->stream>>>(P, c->tri, c->spec);
     else k_tridiag<false><<<gt, 128, 0, c->stream>>>(P, c->tri, c->spec);
-    FZ_LAUNCHED("k_tridiag");
+    FZ_LAUNCHED(FZK_TRI);
+    FZ_TB(FZK_GAUGE);
     k_gauge<<<1, 256, 0, c->stream>>>(P, c->spec, c->M);
-    FZ_LAUNCHED("k_gauge");
+    FZ_LAUNCHED(FZK_GAUGE);
+    FZ_TB(FZK_FFTY_INV);
     k_ffty<+1><<<gy, ty, c->smem_y, c->stream>>>(P, c->spec, c->twy, c->log2ny, c->Sy);
-    FZ_LAUNCHED("k_ffty<+1>");
+    FZ_LAUNCHED(FZK_FFTY_INV);
     const long long nlines = (long long)P.ny * P.nz;
     const unsigned gx = (unsigned)((nlines + 2 * c->Sx - 1) / (2 * c->Sx));
+    FZ_TB(FZK_FFTX_INV);
     k_fftx_inv<<<gx, tx, c->smem_x, c->stream>>>(P, c->spec, dst, 1.0 / ((double)P.nx * (double)P.ny), c->twx,
                                                  c->log2nx, c->Sx);
-    FZ_LAUNCHED("k_fftx_inv");
+    FZ_LAUNCHED(FZK_FFTX_INV);
     return FIZZY_OK;
 }
 
@@ -349,14 +422,16 @@ extern "C" fizzy_status fizzy_set_fields(fizzy_ctx *c, const double *u, const do
     for (double *h : hist)
         if (h) FZ_CUDA(cudaMemsetAsync(h, 0, B, c->stream));
     if (c->P.z_wall) {
+        FZ_TB(FZK_OTHER);
         k_zero_plane<<<(unsigned)((c->P.sxy + 255) / 256), 256, 0, c->stream>>>(c->P, c->w);
-        FZ_LAUNCHED("k_zero_plane");
+        FZ_LAUNCHED(FZK_OTHER);
     }
     const double init[2] = {0.0, c->P.gamma_abs};
     FZ_CUDA(cudaMemcpyAsync(c->scal, init, sizeof(init), cudaMemcpyHostToDevice, c->stream));
     FZ_CUDA(cudaStreamSynchronize(c->stream));  // `init` is a stack variable
+    FZ_TB(FZK_OTHER);
     k_absmax3<<<148 * 8, 256, 0, c->stream>>>(c->P, c->u, c->v, c->w, c->scal);
-    FZ_LAUNCHED("k_absmax3");
+    FZ_LAUNCHED(FZK_OTHER);
     fizzy_status s = run_interface(c);
     if (s != FIZZY_OK) return s;
     c->fields_set = 1;
@@ -390,20 +465,23 @@ extern "C" fizzy_status fizzy_rk3_substep(fizzy_ctx *c, int stage, double dt)
 
     // S0: latch Gamma = gamma_rel * max|u| + gamma_abs (N15)
     if (stage == 0) {
+        FZ_TB(FZK_LATCH);
         k_latch_gamma<<<1, 1, 0, c->stream>>>(P, c->scal);
-        FZ_LAUNCHED("k_latch_gamma");
+        FZ_LAUNCHED(FZK_LATCH);
     }
     // S1: phi transport (divRn holds D(R/Gamma) of the current phi)
+    FZ_TB(FZK_PHI);
     k_phi_update<<<grid, block, 0, c->stream>>>(P, c->phi, c->u, c->v, c->w, c->divrn, c->hphi, c->phin, c->scal,
                                                 dt, gs, zs);
-    FZ_LAUNCHED("k_phi_update");
+    FZ_LAUNCHED(FZK_PHI);
     std::swap(c->phi, c->phin);
     // interface quantities of phi_new (N6): used by S3 now and by S1 of the next substep
     if ((s = run_interface(c)) != FIZZY_OK) return s;
     // S2b: temperature
     if (c->heat) {
+        FZ_TB(FZK_TEMP);
         k_temp_update<<<grid, block, 0, c->stream>>>(P, c->T, c->phi, c->u, c->v, c->w, c->hT, c->Tn, dt, gs, zs);
-        FZ_LAUNCHED("k_temp_update");
+        FZ_LAUNCHED(FZK_TEMP);
         std::swap(c->T, c->Tn);
     }
     // S2 + S3: property map on the fly, momentum predictor -> u**
@@ -412,25 +490,28 @@ extern "C" fizzy_status fizzy_rk3_substep(fizzy_ctx *c, int stage, double dt)
     A.rnx = c->rnx; A.rny = c->rny; A.rnz = c->rnz; A.p = c->p; A.pp = c->pp; A.T = c->T;
     A.us = c->us; A.vs = c->vs; A.ws = c->ws; A.hu = c->hu; A.hv = c->hv; A.hw = c->hw;
     A.scal = c->scal; A.dt = dt; A.gs = gs; A.zs = zs; A.adt = as * dt;
+    FZ_TB(FZK_MOM);
     if (c->varrho) { if (c->varmu) launch_momentum<true, true>(c, grid, block, A); else launch_momentum<true, false>(c, grid, block, A); }
     else { if (c->varmu) launch_momentum<false, true>(c, grid, block, A); else launch_momentum<false, false>(c, grid, block, A); }
-    FZ_LAUNCHED("k_momentum");
+    FZ_LAUNCHED(FZK_MOM);
     // S4: b = rho0/(a dt) D(u**), FFT x (fused), FFT y, tridiagonal z, inverse
     const long long nlines = (long long)P.ny * P.nz;
     const unsigned gx = (unsigned)((nlines + 2 * c->Sx - 1) / (2 * c->Sx));
+    FZ_TB(FZK_FFTX_FWD);
     k_fftx_fwd<true><<<gx, c->Sx * P.nx / 8, c->smem_x, c->stream>>>(P, nullptr, c->us, c->vs, c->ws,
                                                                      P.rho0 / (as * dt), c->spec, c->twx,
                                                                      c->log2nx, c->Sx);
-    FZ_LAUNCHED("k_fftx_fwd");
+    FZ_LAUNCHED(FZK_FFTX_FWD);
     if ((s = run_spectral_solve(c, c->pn)) != FIZZY_OK) return s;
     // S5: correction, pressure rotation
+    FZ_TB(FZK_CORRECT);
     if (stage == 2)
         k_correct<true><<<grid, block, 0, c->stream>>>(P, c->us, c->vs, c->ws, c->pn, c->u, c->v, c->w,
                                                        as * dt / P.rho0, c->scal);
     else
         k_correct<false><<<grid, block, 0, c->stream>>>(P, c->us, c->vs, c->ws, c->pn, c->u, c->v, c->w,
                                                         as * dt / P.rho0, c->scal);
-    FZ_LAUNCHED("k_correct");
+    FZ_LAUNCHED(FZK_CORRECT);
     double *old_pp = c->pp;
     c->pp = c->p;
     c->p = c->pn;
@@ -448,9 +529,10 @@ extern "C" fizzy_status fizzy_poisson_solve(fizzy_ctx *c, const double *rhs, dou
     FZ_CUDA(cudaMemcpyAsync(c->pn, rhs, B, cudaMemcpyDefault, c->stream));
     const long long nlines = (long long)P.ny * P.nz;
     const unsigned gx = (unsigned)((nlines + 2 * c->Sx - 1) / (2 * c->Sx));
+    FZ_TB(FZK_FFTX_FWD);
     k_fftx_fwd<false><<<gx, c->Sx * P.nx / 8, c->smem_x, c->stream>>>(P, c->pn, nullptr, nullptr, nullptr, 1.0,
                                                                       c->spec, c->twx, c->log2nx, c->Sx);
-    FZ_LAUNCHED("k_fftx_fwd<false>");
+    FZ_LAUNCHED(FZK_FFTX_FWD);
     fizzy_status s = run_spectral_solve(c, c->pn);
     if (s != FIZZY_OK) return s;
     FZ_CUDA(cudaMemcpyAsync(p, c->pn, B, cudaMemcpyDefault, c->stream));

@@ -1,0 +1,146 @@
+"""GPU parity: libfizzy.so (through the C ABI, via the ctypes binding) against the CPU oracle on
+the same seeded inputs, element by element.  Tolerances are the ones BASELINE.json:5 states:
+max relative error per field <= 1e-10 after one substep and <= 1e-8 after 10 full RK3 steps,
+with the error norm of reading N19 (max|a-b| / max|b| per field).
+
+Cases are small versions of the five BASELINE.json configs (same recipe and parameters,
+paper_2502_04189_b200.workloads) that the oracle finishes in seconds; they span several
+CTAs / tiles in every kernel, nx != ny != nz, nz not a power of two, periodic / wall /
+stretched-wall z, rho and mu ratios 1, 10 and 1000, heat on and off."""
+import numpy as np
+import pytest
+
+from paper_2502_04189_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+TOL_SUBSTEP = 1e-10
+TOL_10STEPS = 1e-8
+
+CASES = {
+    "cfg0_static_drop_32": lambda: W.make(0),
+    "cfg1_taylor_green_64": lambda: W.make(1, grid=(64, 64, 64), ndrops=2),
+    "cfg2_bubbles_walls_64x64x48": lambda: W.make(2, grid=(64, 64, 48), ndrops=1, radius=0.2),
+    "cfg3_hit_64x32x48": lambda: W.make(3, grid=(64, 32, 48), ndrops=3, radius=0.5),
+    "cfg4_channel_heat_64x32x48": lambda: W.make(4, grid=(64, 32, 48), ndrops=2, radius=0.3),
+    "cfg1_ragged_16x8x5": lambda: W.make(1, grid=(16, 8, 5), ndrops=1, radius=0.8),
+    "cfg4_nx128_ny16": lambda: W.make(4, grid=(128, 16, 12), ndrops=1, radius=0.3),
+}
+
+
+def field_error(a, b):
+    """N19: max|a-b| / max|b|; absolute if the oracle field vanishes."""
+    m = np.abs(b).max()
+    d = np.abs(a - b).max()
+    return d / m if m > 1e-300 else d
+
+
+@pytest.fixture(scope="module")
+def fz():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("GPU test selected but no CUDA device is visible")
+    from paper_2502_04189_b200 import binding
+    return binding
+
+
+def _pair(fz, oracle_mod, name):
+    cfg, f, dt, _ = CASES[name]()
+    o = oracle_mod.Oracle(cfg)
+    o.set_fields(**f)
+    g = fz.Fizzy(cfg)
+    g.set_fields_numpy(**f)
+    return cfg, f, dt, o, g
+
+
+@pytest.mark.parametrize("name", list(CASES))
+def test_one_substep_each_stage(fz, oracle_mod, name):
+    """After each of the first three substeps every field matches the oracle to 1e-10."""
+    cfg, f, dt, o, g = _pair(fz, oracle_mod, name)
+    for stage in range(3):
+        o.substep(stage, dt)
+        g.fizzy_rk3_substep(stage, dt)
+        fo, fg = o.get_fields(), g.get_fields_numpy()
+        for k in fo:
+            assert np.isfinite(fg[k]).all(), (name, stage, k)
+            assert field_error(fg[k], fo[k]) <= TOL_SUBSTEP, (name, stage, k, field_error(fg[k], fo[k]))
+        assert abs(g.fizzy_gamma() - o.gamma()) <= 1e-12 * max(1.0, abs(o.gamma()))
+    g.close()
+
+
+@pytest.mark.parametrize("name", ["cfg0_static_drop_32", "cfg1_taylor_green_64", "cfg2_bubbles_walls_64x64x48",
+                                  "cfg3_hit_64x32x48", "cfg4_channel_heat_64x32x48"])
+def test_ten_steps(fz, oracle_mod, name):
+    """After 10 full RK3 steps every field matches the oracle to 1e-8 (BASELINE.json:5)."""
+    cfg, f, dt, o, g = _pair(fz, oracle_mod, name)
+    for _ in range(10):
+        o.step(dt)
+        g.step(dt)
+    fo, fg = o.get_fields(), g.get_fields_numpy()
+    for k in fo:
+        assert field_error(fg[k], fo[k]) <= TOL_10STEPS, (name, k, field_error(fg[k], fo[k]))
+    g.close()
+
+
+@pytest.mark.parametrize("name", list(CASES))
+def test_poisson_solve(fz, oracle_mod, name):
+    """fizzy_poisson_solve against the oracle's FFT/tridiagonal solver on a random right-hand
+    side (the gauge rule N17 makes the result unique), host pointers in and out."""
+    cfg, f, dt, o, g = _pair(fz, oracle_mod, name)
+    rhs = np.random.default_rng(7).standard_normal(o.shape)
+    po = o.poisson_solve(rhs)
+    pg = np.empty(o.shape)
+    g.fizzy_poisson_solve(np.ascontiguousarray(rhs), pg)
+    g.stream.synchronize()
+    assert field_error(pg, po) <= TOL_SUBSTEP
+    g.close()
+
+
+def test_device_pointers_and_state_errors(fz):
+    """set/get with device tensors; stage order and argument errors come back as status codes."""
+    import torch
+    cfg, f, dt, _ = CASES["cfg0_static_drop_32"]()
+    g = fz.Fizzy(cfg)
+    with pytest.raises(fz.FizzyError) as e:
+        g.fizzy_rk3_substep(0, dt)
+    assert e.value.status == fz.FIZZY_ESTATE
+    dev = {k: torch.from_numpy(v).cuda() for k, v in f.items()}
+    g.fizzy_set_fields(**dev)
+    with pytest.raises(fz.FizzyError) as e:
+        g.fizzy_rk3_substep(1, dt)
+    assert e.value.status == fz.FIZZY_ESTATE
+    with pytest.raises(fz.FizzyError) as e:
+        g.fizzy_rk3_substep(0, -1.0)
+    assert e.value.status == fz.FIZZY_EINVAL
+    out = torch.empty_like(dev["phi"])
+    g.fizzy_get_fields(phi=out)
+    torch.cuda.synchronize()
+    assert torch.equal(out, dev["phi"])
+    n0 = g.fizzy_launch_count()
+    g.step(dt)
+    assert g.fizzy_launch_count() - n0 >= 3 * 10
+    bad = dict(cfg)
+    bad["nx"] = 24
+    with pytest.raises(fz.FizzyError):
+        fz.Fizzy(bad)
+    g.close()
+
+
+def test_properties_at_128(fz):
+    """Properties that hold at any size, on config 2 (BASELINE.json:8) at its full 128^3:
+    projected velocity divergence-free (N20), sum(phi) conserved, phi bounded."""
+    cfg, f, dt, _ = W.make(1)
+    g = fz.Fizzy(cfg)
+    g.set_fields_numpy(**f)
+    for _ in range(3):
+        g.step(dt)
+    out = g.get_fields_numpy()
+    dx, dy, dz = cfg["lx"] / cfg["nx"], cfg["ly"] / cfg["ny"], cfg["lz"] / cfg["nz"]
+    div = ((out["u"] - np.roll(out["u"], 1, 2)) / dx + (out["v"] - np.roll(out["v"], 1, 1)) / dy +
+           (out["w"] - np.roll(out["w"], 1, 0)) / dz)
+    umax = max(np.abs(out[k]).max() for k in "uvw")
+    assert np.abs(div).max() * min(dx, dy, dz) / max(umax, 1.0) <= 1e-12
+    m0 = f["phi"].sum()
+    assert abs(out["phi"].sum() - m0) <= 1e-12 * m0
+    assert out["phi"].min() >= -1e-6 and out["phi"].max() <= 1 + 1e-6
+    g.close()

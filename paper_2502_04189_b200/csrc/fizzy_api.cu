@@ -235,8 +235,10 @@ extern "C" fizzy_status fizzy_create(const fizzy_grid *grid, const fizzy_bc *bc,
     c->N = P.N; c->M = (long long)P.nxh * ny;
     c->varrho = P.rho1 != P.rho2; c->varmu = P.mu1 != P.mu2; c->heat = P.heat != 0; c->cyclic = !bc->z_wall;
     c->log2nx = ilog2(nx); c->log2ny = ilog2(ny);
-    c->Sx = nx >= 1024 ? 4 : (nx >= 32 ? 8 : 256 / nx);   // 1024-point lines: 512 threads per CTA
-    c->Sy = ny >= 1024 ? 4 : (ny >= 32 ? 8 : 256 / ny);
+    // S lines side by side per CTA: 256 threads for n <= 512, 512 threads for n = 1024
+    auto pick_s = [](int n) { return n >= 1024 ? 4 : (n >= 256 ? 2048 / n : (n >= 32 ? 8 : 256 / n)); };
+    c->Sx = pick_s(nx);
+    c->Sy = pick_s(ny);
     c->smem_x = (size_t)nx * (c->Sx + 1) * sizeof(double2);
     c->smem_y = (size_t)ny * (c->Sy + 1) * sizeof(double2);
 
@@ -397,11 +399,31 @@ fizzy_status run_spectral_solve(fizzy_ctx *c, double *dst)
     return FIZZY_OK;
 }
 
-template <bool VR, bool VM>
-void launch_momentum(fizzy_ctx *c, dim3 grid, dim3 block, const FzMomArgs &A)
+template <bool VR, bool VM, bool HT>
+cudaError_t launch_momentum3(fizzy_ctx *c, dim3 grid, dim3 block, const FzMomArgs &A)
 {
-    if (c->heat) k_momentum<VR, VM, true><<<grid, block, 0, c->stream>>>(c->P, A);
-    else k_momentum<VR, VM, false><<<grid, block, 0, c->stream>>>(c->P, A);
+    const FzP &P = c->P;
+    if (P.nx >= MTX && P.ny >= MTY) {   // 2.5-D marching kernel
+        const size_t smem = (size_t)FzMomFields<VR, HT>::NF * MRING * MPS * sizeof(double);
+        cudaError_t e = cudaFuncSetAttribute(k_momentum_march<VR, VM, HT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        const int tiles = (P.nx / MTX) * (P.ny / MTY);
+        int chunks = 8192 / tiles;
+        if (chunks > P.nz / 16) chunks = P.nz / 16;
+        if (chunks < 1) chunks = 1;
+        const int KC = (P.nz + chunks - 1) / chunks;
+        const dim3 g(P.nx / MTX, P.ny / MTY, (P.nz + KC - 1) / KC);
+        k_momentum_march<VR, VM, HT><<<g, dim3(MTX, MTY), smem, c->stream>>>(P, A, KC);
+    } else {                            // tiny grids: one thread per cell straight from global memory
+        k_momentum<VR, VM, HT><<<grid, block, 0, c->stream>>>(P, A);
+    }
+    return cudaSuccess;
+}
+
+template <bool VR, bool VM>
+cudaError_t launch_momentum(fizzy_ctx *c, dim3 grid, dim3 block, const FzMomArgs &A)
+{
+    return c->heat ? launch_momentum3<VR, VM, true>(c, grid, block, A) : launch_momentum3<VR, VM, false>(c, grid, block, A);
 }
 
 }  // namespace

@@ -122,7 +122,7 @@ __device__ __forceinline__ void fz_fft_tile(double2 *sm, const double2 *__restri
 //   b = coef * D(u**)  (BASELINE.json:5(iv) with the p_hat term folded into u**, D2);
 // DIV = false: the real input is read from `src` (fizzy_poisson_solve).
 template <bool DIV>
-__global__ void k_fftx_fwd(FzP P, const double *__restrict__ src, const double *__restrict__ us,
+__global__ void __launch_bounds__(512, 2) k_fftx_fwd(FzP P, const double *__restrict__ src, const double *__restrict__ us,
                            const double *__restrict__ vs, const double *__restrict__ ws, double coef,
                            double2 *__restrict__ spec, const double2 *__restrict__ tw, int log2n, int S)
 {
@@ -174,7 +174,7 @@ __global__ void k_fftx_fwd(FzP P, const double *__restrict__ src, const double *
 
 // ---------------------------------------------------------------- FFT along x, backward (c2r)
 // Z_l = A_l + i B_l, Z_{n-l} = conj(A_l) + i conj(B_l); out = Re/Im of the inverse transform * scale
-__global__ void k_fftx_inv(FzP P, const double2 *__restrict__ spec, double *__restrict__ dst, double scale,
+__global__ void __launch_bounds__(512, 2) k_fftx_inv(FzP P, const double2 *__restrict__ spec, double *__restrict__ dst, double scale,
                            const double2 *__restrict__ tw, int log2n, int S)
 {
     extern __shared__ double2 sm[];
@@ -211,7 +211,7 @@ __global__ void k_fftx_inv(FzP P, const double2 *__restrict__ spec, double *__re
 // ---------------------------------------------------------------- FFT along y (complex, in place)
 // CTA = (block of S consecutive l, plane k); element m of slot s is spec[(k*ny + m)*nxh + l0 + s].
 template <int SGN>
-__global__ void k_ffty(FzP P, double2 *__restrict__ spec, const double2 *__restrict__ tw, int log2n, int S)
+__global__ void __launch_bounds__(512, 2) k_ffty(FzP P, double2 *__restrict__ spec, const double2 *__restrict__ tw, int log2n, int S)
 {
     extern __shared__ double2 sm[];
     const int n = P.ny, LP = S + 1, nxh = P.nxh;

@@ -186,3 +186,255 @@ k_momentum(FzP P, FzMomArgs A)
         A.hw[c] = 0.0;
     }
 }
+
+// =====================================================================================
+// 2.5-D marching variant (the one used when nx >= 32 and ny >= 8).  A CTA owns an x-y tile of
+// MTX x MTY cells and marches over a chunk of z planes.  Every staged field keeps a ring of four
+// planes (tile + halo 1) in shared memory, so each plane is read from HBM once per chunk, all
+// 60-odd neighbour reads of the stencil are shared-memory reads, and the global loads of plane
+// k+2 are issued before the arithmetic of plane k (software prefetch through registers): DRAM
+// latency is hidden by the pipeline rather than by occupancy.  One barrier per plane: with four
+// slots the plane written at step k (k+1) is never one that a lagging warp may still read
+// (k-2 .. k).  Wall ghosts (no-slip: -u, -v; impermeable: w = 0, R_z = 0; mirror: phi, kappa,
+// p_hat; Dirichlet: 2 T_wall - T) are applied when a ghost plane is written into the ring.
+#define MTX 32
+#define MTY 8
+#define MPW (MTX + 2)
+#define MPH (MTY + 2)
+#define MPS (MPW * MPH)
+#define MRING 4
+#define MHALO (MPS - MTX * MTY)
+
+template <bool VARRHO, bool HEAT>
+struct FzMomFields {
+    static constexpr int U = 0, V = 1, W = 2, PHI = 3, KAP = 4;
+    static constexpr int T = 5;                        // valid if HEAT
+    static constexpr int RX = 5 + (HEAT ? 1 : 0);      // valid if VARRHO
+    static constexpr int RY = RX + 1, RZ = RX + 2, PH = RX + 3;
+    static constexpr int NF = 5 + (HEAT ? 1 : 0) + (VARRHO ? 4 : 0);
+};
+
+template <bool VARRHO, bool VARMU, bool HEAT>
+__global__ void __launch_bounds__(MTX * MTY)
+k_momentum_march(FzP P, FzMomArgs A, int KC)
+{
+    using F = FzMomFields<VARRHO, HEAT>;
+    constexpr int NF = F::NF;
+    extern __shared__ double smm[];  // [NF][MRING][MPS]
+    const int tx = threadIdx.x, ty = threadIdx.y, t = ty * MTX + tx;
+    const int i0 = blockIdx.x * MTX, j0 = blockIdx.y * MTY;
+    const int i = i0 + tx, j = j0 + ty;
+    const int k0 = blockIdx.z * KC, k1 = min(k0 + KC, P.nz);
+    const int cidx = (ty + 1) * MPW + (tx + 1);
+    // this thread's halo point (threads 0..MHALO-1): top row, bottom row, left column, right column
+    int hx = 0, hy = 0;
+    if (t < MPW) { hx = t - 1; hy = -1; }
+    else if (t < 2 * MPW) { hx = t - MPW - 1; hy = MTY; }
+    else if (t < 2 * MPW + MTY) { hx = -1; hy = t - 2 * MPW; }
+    else { hx = MTX; hy = t - 2 * MPW - MTY; }
+    const bool has_halo = t < MHALO;
+    const int hidx = (hy + 1) * MPW + (hx + 1);
+    const long long goff_c = i + (long long)P.nx * j;
+    const long long goff_h = ((i0 + hx + P.nx) & (P.nx - 1)) + (long long)P.nx * ((j0 + hy + P.ny) & (P.ny - 1));
+
+    const double *src[NF];
+    src[F::U] = A.u; src[F::V] = A.v; src[F::W] = A.w; src[F::PHI] = A.phi; src[F::KAP] = A.kappa;
+    if (HEAT) src[F::T] = A.T;
+    if (VARRHO) { src[F::RX] = A.rnx; src[F::RY] = A.rny; src[F::RZ] = A.rnz; src[F::PH] = A.p; }
+
+    double rc[NF], rh[NF];
+    // fetch plane kk (k0-1 .. k1) of every staged field into registers, ghost rules applied
+    auto fetch = [&](int kk) {
+        int sp = kk;
+        int ghost = 0;  // -1 bottom wall ghost, +1 top wall ghost
+        if (P.z_wall) {
+            if (kk < 0) { sp = 0; ghost = -1; }
+            else if (kk >= P.nz) { sp = P.nz - 1; ghost = 1; }
+        } else {
+            sp = kk < 0 ? kk + P.nz : (kk >= P.nz ? kk - P.nz : kk);
+        }
+        const long long pc = (long long)sp * P.sxy + goff_c, ph = (long long)sp * P.sxy + goff_h;
+#pragma unroll
+        for (int f = 0; f < NF; ++f) {
+            double a = src[f][pc];
+            double b = has_halo ? src[f][ph] : 0.0;
+            if (VARRHO && f == F::PH) {  // p_hat = 2 p - p_prev (N7)
+                a = 2.0 * a - A.pp[pc];
+                if (has_halo) b = 2.0 * b - A.pp[ph];
+            }
+            if (ghost != 0) {
+                if (f == F::U || f == F::V) { a = -a; b = -b; }
+                else if (f == F::W || (VARRHO && f == F::RZ)) { a = 0.0; b = 0.0; }
+                else if (HEAT && f == F::T) {
+                    const double tw = ghost < 0 ? P.t_bot : P.t_top;
+                    a = 2.0 * tw - a; b = 2.0 * tw - b;
+                }
+            }
+            rc[f] = a; rh[f] = b;
+        }
+    };
+    auto stash = [&](int kk) {
+        const int slot = (kk + MRING) & (MRING - 1);
+#pragma unroll
+        for (int f = 0; f < NF; ++f) {
+            double *pl = smm + (f * MRING + slot) * MPS;
+            pl[cidx] = rc[f];
+            if (has_halo) pl[hidx] = rh[f];
+        }
+    };
+
+    fetch(k0 - 1); stash(k0 - 1);
+    fetch(k0); stash(k0);
+    fetch(k0 + 1);
+
+    const double dx = P.idx, dy = P.idy;
+    const double dmu = P.mu1 - P.mu2;
+    const double ir0 = 1.0 / P.rho0;
+    const double Gam = A.scal[1];
+
+    for (int k = k0; k < k1; ++k) {
+        stash(k + 1);
+        __syncthreads();
+        if (k + 2 <= k1) fetch(k + 2);
+        const long long c = (long long)k * P.sxy + goff_c;
+        const double hu_old = A.hu[c], hv_old = A.hv[c], hw_old = A.hw[c];
+        const int om = ((k - 1 + MRING) & (MRING - 1)) * MPS + cidx, o0 = (k & (MRING - 1)) * MPS + cidx,
+                  op = ((k + 1) & (MRING - 1)) * MPS + cidx;
+        // S(f, di, dj, plane offset) -- shared-memory neighbour read
+#define S_(f, di, dj, o) smm[(f) * (MRING * MPS) + (o) + (dj) * MPW + (di)]
+        const double izf = P.idzf[k], izc = P.idzc[k], izcm = P.idzc[k - 1];
+        const double u000 = S_(F::U, 0, 0, o0), up00 = S_(F::U, 1, 0, o0), um00 = S_(F::U, -1, 0, o0);
+        const double u0p0 = S_(F::U, 0, 1, o0), u0m0 = S_(F::U, 0, -1, o0), ump0 = S_(F::U, -1, 1, o0);
+        const double u00p = S_(F::U, 0, 0, op), u00m = S_(F::U, 0, 0, om), um0p = S_(F::U, -1, 0, op);
+        const double v000 = S_(F::V, 0, 0, o0), vp00 = S_(F::V, 1, 0, o0), vm00 = S_(F::V, -1, 0, o0);
+        const double v0p0 = S_(F::V, 0, 1, o0), v0m0 = S_(F::V, 0, -1, o0), vpm0 = S_(F::V, 1, -1, o0);
+        const double v00p = S_(F::V, 0, 0, op), v00m = S_(F::V, 0, 0, om), v0mp = S_(F::V, 0, -1, op);
+        const double w000 = S_(F::W, 0, 0, o0), wp00 = S_(F::W, 1, 0, o0), wm00 = S_(F::W, -1, 0, o0);
+        const double w0p0 = S_(F::W, 0, 1, o0), w0m0 = S_(F::W, 0, -1, o0);
+        const double w00m = S_(F::W, 0, 0, om), wp0m = S_(F::W, 1, 0, om), w0pm = S_(F::W, 0, 1, om);
+        const double f000 = S_(F::PHI, 0, 0, o0), fp00 = S_(F::PHI, 1, 0, o0), f0p0 = S_(F::PHI, 0, 1, o0),
+                     f00p = S_(F::PHI, 0, 0, op);
+        double m000, mp00, mm00, m0p0, m0m0, m00p, m00m, mpp0, mpm0, mmp0, mp0p, mp0m, mm0p, m0pp, m0pm, m0mp;
+        if (VARMU) {
+#define FZ_MU(x) (P.mu2 + dmu * fz_clip01(x))
+            m000 = FZ_MU(f000); mp00 = FZ_MU(fp00); m0p0 = FZ_MU(f0p0); m00p = FZ_MU(f00p);
+            mm00 = FZ_MU(S_(F::PHI, -1, 0, o0)); m0m0 = FZ_MU(S_(F::PHI, 0, -1, o0)); m00m = FZ_MU(S_(F::PHI, 0, 0, om));
+            mpp0 = FZ_MU(S_(F::PHI, 1, 1, o0)); mpm0 = FZ_MU(S_(F::PHI, 1, -1, o0)); mmp0 = FZ_MU(S_(F::PHI, -1, 1, o0));
+            mp0p = FZ_MU(S_(F::PHI, 1, 0, op)); mp0m = FZ_MU(S_(F::PHI, 1, 0, om)); mm0p = FZ_MU(S_(F::PHI, -1, 0, op));
+            m0pp = FZ_MU(S_(F::PHI, 0, 1, op)); m0pm = FZ_MU(S_(F::PHI, 0, 1, om)); m0mp = FZ_MU(S_(F::PHI, 0, -1, op));
+#undef FZ_MU
+        } else {
+            m000 = mp00 = mm00 = m0p0 = m0m0 = m00p = m00m = mpp0 = mpm0 = mmp0 = mp0p = mp0m = mm0p = m0pp =
+                m0pm = m0mp = P.mu2;
+        }
+        const double kap0 = S_(F::KAP, 0, 0, o0);
+        double irx = 1.0 / P.rho2, iry = irx, irz = irx;
+        double ph000 = 0, php00 = 0, ph0p0 = 0, ph00p = 0;
+        if (VARRHO) {
+            const double r000 = P.rho2 + P.drho * fz_clip01(f000);
+            irx = 1.0 / (0.5 * (r000 + P.rho2 + P.drho * fz_clip01(fp00)));
+            iry = 1.0 / (0.5 * (r000 + P.rho2 + P.drho * fz_clip01(f0p0)));
+            irz = 1.0 / (0.5 * (r000 + P.rho2 + P.drho * fz_clip01(f00p)));
+            ph000 = S_(F::PH, 0, 0, o0); php00 = S_(F::PH, 1, 0, o0); ph0p0 = S_(F::PH, 0, 1, o0);
+            ph00p = S_(F::PH, 0, 0, op);
+        }
+        double T000 = 0;
+        if (HEAT) T000 = S_(F::T, 0, 0, o0);
+        // ================= x component =================
+        {
+            const double uc_p = 0.5 * (up00 + u000), uc_m = 0.5 * (u000 + um00);
+            const double Exy_p = 0.5 * (v000 + vp00) * 0.5 * (u000 + u0p0);
+            const double Exy_m = 0.5 * (v0m0 + vpm0) * 0.5 * (u0m0 + u000);
+            const double Exz_p = 0.5 * (w000 + wp00) * 0.5 * (u000 + u00p);
+            const double Exz_m = 0.5 * (w00m + wp0m) * 0.5 * (u00m + u000);
+            const double Aa = -(uc_p * uc_p - uc_m * uc_m) * dx - (Exy_p - Exy_m) * dy - (Exz_p - Exz_m) * izf;
+            const double nrm_p = 2.0 * mp00 * (up00 - u000) * dx, nrm_m = 2.0 * m000 * (u000 - um00) * dx;
+            const double txy_p = 0.25 * (m000 + mp00 + m0p0 + mpp0) * ((u0p0 - u000) * dy + (vp00 - v000) * dx);
+            const double txy_m = 0.25 * (m0m0 + mpm0 + m000 + mp00) * ((u000 - u0m0) * dy + (vpm0 - v0m0) * dx);
+            const double txz_p = 0.25 * (m000 + mp00 + m00p + mp0p) * ((u00p - u000) * izc + (wp00 - w000) * dx);
+            const double txz_m = 0.25 * (m00m + mp0m + m000 + mp00) * ((u000 - u00m) * izcm + (wp0m - w00m) * dx);
+            const double V = (nrm_p - nrm_m) * dx + (txy_p - txy_m) * dy + (txz_p - txz_m) * izf;
+            const double Sf = P.sigma * 0.5 * (kap0 + S_(F::KAP, 1, 0, o0)) * (fp00 - f000) * dx;
+            double M = 0.0;
+            if (VARRHO) {
+                const double Rty = 0.25 * (S_(F::RY, 0, 0, o0) + S_(F::RY, 1, 0, o0) + S_(F::RY, 0, -1, o0) + S_(F::RY, 1, -1, o0));
+                const double Rtz = 0.25 * (S_(F::RZ, 0, 0, o0) + S_(F::RZ, 1, 0, o0) + S_(F::RZ, 0, 0, om) + S_(F::RZ, 1, 0, om));
+                M = P.drho * Gam * (S_(F::RX, 0, 0, o0) * (up00 - um00) * (0.5 * dx) + Rty * (u0p0 - u0m0) * (0.5 * dy) +
+                                    Rtz * (u00p - u00m) * P.igz[k]);
+            }
+            double B = P.gx * (1.0 - P.rho_ref * irx) + P.fx + P.a_lin * u000;
+            if (HEAT) B -= P.gx * P.beta * (0.5 * (T000 + S_(F::T, 1, 0, o0)) - P.t_ref);
+            const double rhs = Aa + (V + Sf + M) * irx + B;
+            double un = u000 + A.dt * (A.gs * rhs + A.zs * hu_old);
+            if (VARRHO) un -= A.adt * (irx - ir0) * (php00 - ph000) * dx;
+            A.us[c] = un;
+            A.hu[c] = rhs;
+        }
+        // ================= y component =================
+        {
+            const double vc_p = 0.5 * (v0p0 + v000), vc_m = 0.5 * (v000 + v0m0);
+            const double Eyx_p = 0.5 * (u000 + u0p0) * 0.5 * (v000 + vp00);
+            const double Eyx_m = 0.5 * (um00 + ump0) * 0.5 * (vm00 + v000);
+            const double Eyz_p = 0.5 * (w000 + w0p0) * 0.5 * (v000 + v00p);
+            const double Eyz_m = 0.5 * (w00m + w0pm) * 0.5 * (v00m + v000);
+            const double Aa = -(vc_p * vc_p - vc_m * vc_m) * dy - (Eyx_p - Eyx_m) * dx - (Eyz_p - Eyz_m) * izf;
+            const double nrm_p = 2.0 * m0p0 * (v0p0 - v000) * dy, nrm_m = 2.0 * m000 * (v000 - v0m0) * dy;
+            const double tyx_p = 0.25 * (m000 + m0p0 + mp00 + mpp0) * ((vp00 - v000) * dx + (u0p0 - u000) * dy);
+            const double tyx_m = 0.25 * (mm00 + mmp0 + m000 + m0p0) * ((v000 - vm00) * dx + (ump0 - um00) * dy);
+            const double tyz_p = 0.25 * (m000 + m0p0 + m00p + m0pp) * ((v00p - v000) * izc + (w0p0 - w000) * dy);
+            const double tyz_m = 0.25 * (m00m + m0pm + m000 + m0p0) * ((v000 - v00m) * izcm + (w0pm - w00m) * dy);
+            const double V = (nrm_p - nrm_m) * dy + (tyx_p - tyx_m) * dx + (tyz_p - tyz_m) * izf;
+            const double Sf = P.sigma * 0.5 * (kap0 + S_(F::KAP, 0, 1, o0)) * (f0p0 - f000) * dy;
+            double M = 0.0;
+            if (VARRHO) {
+                const double Rtx = 0.25 * (S_(F::RX, 0, 0, o0) + S_(F::RX, 0, 1, o0) + S_(F::RX, -1, 0, o0) + S_(F::RX, -1, 1, o0));
+                const double Rtz = 0.25 * (S_(F::RZ, 0, 0, o0) + S_(F::RZ, 0, 1, o0) + S_(F::RZ, 0, 0, om) + S_(F::RZ, 0, 1, om));
+                M = P.drho * Gam * (S_(F::RY, 0, 0, o0) * (v0p0 - v0m0) * (0.5 * dy) + Rtx * (vp00 - vm00) * (0.5 * dx) +
+                                    Rtz * (v00p - v00m) * P.igz[k]);
+            }
+            double B = P.gy * (1.0 - P.rho_ref * iry) + P.fy + P.a_lin * v000;
+            if (HEAT) B -= P.gy * P.beta * (0.5 * (T000 + S_(F::T, 0, 1, o0)) - P.t_ref);
+            const double rhs = Aa + (V + Sf + M) * iry + B;
+            double vn = v000 + A.dt * (A.gs * rhs + A.zs * hv_old);
+            if (VARRHO) vn -= A.adt * (iry - ir0) * (ph0p0 - ph000) * dy;
+            A.vs[c] = vn;
+            A.hv[c] = rhs;
+        }
+        // ================= z component =================
+        if (k < P.kzf) {
+            const double w00p = S_(F::W, 0, 0, op);
+            const double izfp = P.idzf[k + 1];
+            const double wc_p = 0.5 * (w00p + w000), wc_m = 0.5 * (w000 + w00m);
+            const double Ezx_p = 0.5 * (u000 + u00p) * 0.5 * (w000 + wp00);
+            const double Ezx_m = 0.5 * (um00 + um0p) * 0.5 * (wm00 + w000);
+            const double Ezy_p = 0.5 * (v000 + v00p) * 0.5 * (w000 + w0p0);
+            const double Ezy_m = 0.5 * (v0m0 + v0mp) * 0.5 * (w0m0 + w000);
+            const double Aa = -(wc_p * wc_p - wc_m * wc_m) * izc - (Ezx_p - Ezx_m) * dx - (Ezy_p - Ezy_m) * dy;
+            const double nrm_p = 2.0 * m00p * (w00p - w000) * izfp, nrm_m = 2.0 * m000 * (w000 - w00m) * izf;
+            const double tzx_p = 0.25 * (m000 + m00p + mp00 + mp0p) * ((wp00 - w000) * dx + (u00p - u000) * izc);
+            const double tzx_m = 0.25 * (mm00 + mm0p + m000 + m00p) * ((w000 - wm00) * dx + (um0p - um00) * izc);
+            const double tzy_p = 0.25 * (m000 + m00p + m0p0 + m0pp) * ((w0p0 - w000) * dy + (v00p - v000) * izc);
+            const double tzy_m = 0.25 * (m0m0 + m0mp + m000 + m00p) * ((w000 - w0m0) * dy + (v0mp - v0m0) * izc);
+            const double V = (nrm_p - nrm_m) * izc + (tzx_p - tzx_m) * dx + (tzy_p - tzy_m) * dy;
+            const double Sf = P.sigma * 0.5 * (kap0 + S_(F::KAP, 0, 0, op)) * (f00p - f000) * izc;
+            double M = 0.0;
+            if (VARRHO) {
+                const double Rtx = 0.25 * (S_(F::RX, 0, 0, o0) + S_(F::RX, 0, 0, op) + S_(F::RX, -1, 0, o0) + S_(F::RX, -1, 0, op));
+                const double Rty = 0.25 * (S_(F::RY, 0, 0, o0) + S_(F::RY, 0, 0, op) + S_(F::RY, 0, -1, o0) + S_(F::RY, 0, -1, op));
+                M = P.drho * Gam * (S_(F::RZ, 0, 0, o0) * (w00p - w00m) / (P.dzf[k + 1] + P.dzf[k]) +
+                                    Rtx * (wp00 - wm00) * (0.5 * dx) + Rty * (w0p0 - w0m0) * (0.5 * dy));
+            }
+            double B = P.gz * (1.0 - P.rho_ref * irz) + P.fz + P.a_lin * w000;
+            if (HEAT) B -= P.gz * P.beta * (0.5 * (T000 + S_(F::T, 0, 0, op)) - P.t_ref);
+            const double rhs = Aa + (V + Sf + M) * irz + B;
+            double wn = w000 + A.dt * (A.gs * rhs + A.zs * hw_old);
+            if (VARRHO) wn -= A.adt * (irz - ir0) * (ph00p - ph000) * izc;
+            A.ws[c] = wn;
+            A.hw[c] = rhs;
+        } else {
+            A.ws[c] = 0.0;
+            A.hw[c] = 0.0;
+        }
+#undef S_
+    }
+}

@@ -198,9 +198,18 @@ __global__ void k_correct(FzP P, const double *__restrict__ us, const double *__
     v[c] = vn;
     w[c] = wn;
     if (WITH_MAX) {
+        // block max, then at most one atomic per CTA (and none if the running max is already larger)
+        __shared__ double wmax[8];
         double m = fmax(fabs(un), fmax(fabs(vn), fabs(wn)));
         for (int o = 16; o > 0; o >>= 1) m = fmax(m, __shfl_xor_sync(0xffffffffu, m, o));
-        if (((threadIdx.x + blockDim.x * threadIdx.y) & 31) == 0) fz_atomic_max_nonneg(umax, m);
+        const int t = threadIdx.x + blockDim.x * threadIdx.y;
+        if ((t & 31) == 0) wmax[t >> 5] = m;
+        __syncthreads();
+        if (t == 0) {
+            const int nw = (blockDim.x * blockDim.y + 31) >> 5;
+            for (int q = 1; q < nw; ++q) m = fmax(m, wmax[q]);
+            if (m > *reinterpret_cast<volatile double *>(umax)) fz_atomic_max_nonneg(umax, m);
+        }
     }
 }
 

@@ -40,9 +40,8 @@ def algorithmic_bytes_per_cell(cfg):
     varrho = cfg["rho1"] != cfg["rho2"]
     heat = bool(cfg["heat"])
     b = {
-        "k_phi_update": 64.0,                                   # r phi,u,v,w,hphi,divRn  w phi,hphi
-        "k_iface_psi": 24.0, "k_iface_nhat": 32.0,              # interface kernels (group a)
-        "k_iface_flux": 56.0 + (24.0 if varrho else 0.0),
+        "k_phi_update": 80.0,                                   # r phi,u,v,w,hphi,divRn  w phi,hphi,psi,r
+        "k_iface_march": 40.0 + (24.0 if varrho else 0.0),      # r psi,r,phi  w kappa,divRn (+Rn x3)
         "k_momentum": 112.0 + (40.0 if varrho else 0.0) + (8.0 if heat else 0.0),
         "k_fftx_fwd": 24.0 + spec, "k_ffty_fwd": 2 * spec, "k_tridiag": 2 * spec,
         "k_ffty_inv": 2 * spec, "k_fftx_inv": spec + 8.0, "k_correct": 56.0,

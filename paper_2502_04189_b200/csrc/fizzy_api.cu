@@ -11,6 +11,7 @@
 
 #include "fz_common.cuh"
 #include "fz_fft.cuh"
+#include "fz_iface.cuh"
 #include "fz_momentum.cuh"
 #include "fz_stencil.cuh"
 #include "fz_tridiag.cuh"
@@ -35,10 +36,10 @@ struct Carver {  // hands out 256-byte aligned pieces of the workspace (or just 
 
 }  // namespace
 
-enum FzKernelId { FZK_LATCH, FZK_PHI, FZK_IPSI, FZK_INHAT, FZK_IFLUX, FZK_TEMP, FZK_MOM, FZK_FFTX_FWD,
+enum FzKernelId { FZK_LATCH, FZK_PHI, FZK_IMARCH, FZK_IPSI, FZK_INHAT, FZK_IFLUX, FZK_TEMP, FZK_MOM, FZK_FFTX_FWD,
                   FZK_FFTY_FWD, FZK_TRI, FZK_GAUGE, FZK_FFTY_INV, FZK_FFTX_INV, FZK_CORRECT, FZK_OTHER, FZK_COUNT };
 static const char *const FZK_NAME[FZK_COUNT] = {
-    "k_latch_gamma", "k_phi_update", "k_iface_psi", "k_iface_nhat", "k_iface_flux", "k_temp_update", "k_momentum",
+    "k_latch_gamma", "k_phi_update", "k_iface_march", "k_iface_psi", "k_iface_nhat", "k_iface_flux", "k_temp_update", "k_momentum",
     "k_fftx_fwd", "k_ffty_fwd", "k_tridiag", "k_gauge", "k_ffty_inv", "k_fftx_inv", "k_correct", "other"};
 
 struct FzTimed { int id; cudaEvent_t e0, e1; };
@@ -287,6 +288,8 @@ extern "C" fizzy_status fizzy_create(const fizzy_grid *grid, const fizzy_bc *bc,
     FZ_LAUNCHED(FZK_OTHER);
 
     // dynamic shared memory opt-in for the FFT kernels
+    FZ_CUDA(cudaFuncSetAttribute(k_iface_march<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)IFACE_SMEM));
+    FZ_CUDA(cudaFuncSetAttribute(k_iface_march<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)IFACE_SMEM));
     FZ_CUDA(cudaFuncSetAttribute(k_fftx_fwd<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_x));
     FZ_CUDA(cudaFuncSetAttribute(k_fftx_fwd<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_x));
     FZ_CUDA(cudaFuncSetAttribute(k_fftx_inv, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_x));
@@ -348,14 +351,36 @@ extern "C" double fizzy_gamma(fizzy_ctx *c)
 // =====================================================================================
 namespace {
 
-// interface quantities of c->phi -> kappa, divRn (and Rn when rho1 != rho2): kernel group (a)
-fizzy_status run_interface(fizzy_ctx *c)
+// interface quantities of c->phi -> kappa, divRn (and Rn when rho1 != rho2): kernel group (a).
+// with_psi: psi and r = sqrt(q) of c->phi are not yet in c->psi / c->rr (fizzy_set_fields);
+// inside a substep k_phi_update has already written them.
+fizzy_status run_interface(fizzy_ctx *c, bool with_psi)
 {
+    const FzP &P = c->P;
     dim3 grid, block;
     cell_launch(c, grid, block);
-    FZ_TB(FZK_IPSI);
-    k_iface_psi<<<grid, block, 0, c->stream>>>(c->P, c->phi, c->psi, c->rr);
-    FZ_LAUNCHED(FZK_IPSI);
+    if (with_psi) {
+        FZ_TB(FZK_IPSI);
+        k_iface_psi<<<grid, block, 0, c->stream>>>(c->P, c->phi, c->psi, c->rr);
+        FZ_LAUNCHED(FZK_IPSI);
+    }
+    if (P.nx >= ITX && P.ny >= ITY) {   // marching sweep: nhat stays on chip
+        int chunks = 8192 / ((P.nx / ITX) * (P.ny / ITY));
+        if (chunks > P.nz / 16) chunks = P.nz / 16;
+        if (chunks < 1) chunks = 1;
+        const int KC = (P.nz + chunks - 1) / chunks;
+        const dim3 g(P.nx / ITX, P.ny / ITY, (P.nz + KC - 1) / KC);
+        FZ_TB(FZK_IMARCH);
+        if (c->varrho)
+            k_iface_march<true><<<g, dim3(ITX, ITY), IFACE_SMEM, c->stream>>>(P, c->psi, c->rr, c->phi, c->kappa, c->divrn,
+                                                                              c->rnx, c->rny, c->rnz, KC);
+        else
+            k_iface_march<false><<<g, dim3(ITX, ITY), IFACE_SMEM, c->stream>>>(P, c->psi, c->rr, c->phi, c->kappa, c->divrn,
+                                                                               nullptr, nullptr, nullptr, KC);
+        FZ_LAUNCHED(FZK_IMARCH);
+        return FIZZY_OK;
+    }
+    // tiny grids: one thread per cell, nhat through global memory
     FZ_TB(FZK_INHAT);
     k_iface_nhat<<<grid, block, 0, c->stream>>>(c->P, c->psi, c->nhx, c->nhy, c->nhz);
     FZ_LAUNCHED(FZK_INHAT);
@@ -454,7 +479,7 @@ extern "C" fizzy_status fizzy_set_fields(fizzy_ctx *c, const double *u, const do
     FZ_TB(FZK_OTHER);
     k_absmax3<<<148 * 8, 256, 0, c->stream>>>(c->P, c->u, c->v, c->w, c->scal);
     FZ_LAUNCHED(FZK_OTHER);
-    fizzy_status s = run_interface(c);
+    fizzy_status s = run_interface(c, true);
     if (s != FIZZY_OK) return s;
     c->fields_set = 1;
     c->next_stage = 0;
@@ -493,12 +518,12 @@ extern "C" fizzy_status fizzy_rk3_substep(fizzy_ctx *c, int stage, double dt)
     }
     // S1: phi transport (divRn holds D(R/Gamma) of the current phi)
     FZ_TB(FZK_PHI);
-    k_phi_update<<<grid, block, 0, c->stream>>>(P, c->phi, c->u, c->v, c->w, c->divrn, c->hphi, c->phin, c->scal,
+    k_phi_update<<<grid, block, 0, c->stream>>>(P, c->phi, c->u, c->v, c->w, c->divrn, c->hphi, c->phin, c->psi, c->rr, c->scal,
                                                 dt, gs, zs);
     FZ_LAUNCHED(FZK_PHI);
     std::swap(c->phi, c->phin);
     // interface quantities of phi_new (N6): used by S3 now and by S1 of the next substep
-    if ((s = run_interface(c)) != FIZZY_OK) return s;
+    if ((s = run_interface(c, false)) != FIZZY_OK) return s;
     // S2b: temperature
     if (c->heat) {
         FZ_TB(FZK_TEMP);

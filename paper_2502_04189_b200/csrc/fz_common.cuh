@@ -62,3 +62,40 @@ __device__ __forceinline__ double2 fz_cmul(double2 a, double2 b)
 {
     return make_double2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x);
 }
+
+// Branch-free reciprocal and reciprocal square root for NORMAL, finite, positive arguments whose
+// results are normal too (callers guarantee the range): hardware seed (MUFU.RCP64H / RSQ64H, about
+// 2^-22 relative) + two Newton steps -> ~1 ulp.  The IEEE `/` and rsqrt() carry a slow-path branch
+// per call that these stencils never need.
+__device__ __forceinline__ double fz_rcp(double d)
+{
+    double x;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(x) : "d"(d));
+    double e = fma(-d, x, 1.0);
+    x = fma(x, e, x);
+    e = fma(-d, x, 1.0);
+    return fma(x, e, x);
+}
+__device__ __forceinline__ double fz_rsqrt(double a)
+{
+    double y;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(a));
+    const double h = 0.5 * a;
+    double e = fma(-h * y, y, 0.5);   // 0.5 - 0.5 a y^2
+    y = fma(y, e, y);
+    e = fma(-h * y, y, 0.5);
+    return fma(y, e, y);
+}
+
+// 8- and 16-byte asynchronous global -> shared copies (LDGSTS) and their group fences
+__device__ __forceinline__ void fz_cp_async16(void *smem_dst, const void *gsrc)
+{
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((unsigned)__cvta_generic_to_shared(smem_dst)), "l"(gsrc) : "memory");
+}
+__device__ __forceinline__ void fz_cp_async8(void *smem_dst, const void *gsrc)
+{
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"((unsigned)__cvta_generic_to_shared(smem_dst)), "l"(gsrc) : "memory");
+}
+__device__ __forceinline__ void fz_cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void fz_cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }

@@ -115,10 +115,12 @@ __global__ void k_iface_flux(FzP P, const double *__restrict__ phi, const double
 
 // ---------------------------------------------------------------- S1: ACDI phi transport
 // RHSphi = D(-u_a phibar_a) + Gamma D(Rn);  phi <- phi + dt (g RHS + z RHS_old)   (BASELINE.json:5(i))
+// also writes psi = eps ln q and r = sqrt q of phi_new (N2), the inputs of k_iface_march
 __global__ void k_phi_update(FzP P, const double *__restrict__ phi, const double *__restrict__ u,
                              const double *__restrict__ v, const double *__restrict__ w,
                              const double *__restrict__ divrn, double *__restrict__ hphi,
-                             double *__restrict__ phin, const double *__restrict__ scal, double dt,
+                             double *__restrict__ phin, double *__restrict__ psi,
+                             double *__restrict__ rr, const double *__restrict__ scal, double dt,
                              double gs, double zs)
 {
     FZ_CELL_IJK
@@ -134,8 +136,14 @@ __global__ void k_phi_update(FzP P, const double *__restrict__ phi, const double
     const double Fzp = z.gp ? 0.0 : -w[c] * 0.5 * (f0 + phi[zp]);
     const double Fzm = z.gm ? 0.0 : -w[zm] * 0.5 * (phi[zm] + f0);
     const double rhs = (Fxp - Fxm) * P.idx + (Fyp - Fym) * P.idy + (Fzp - Fzm) * P.idzf[k] + scal[1] * divrn[c];
-    phin[c] = f0 + dt * (gs * rhs + zs * hphi[c]);
+    const double fn = f0 + dt * (gs * rhs + zs * hphi[c]);
+    phin[c] = fn;
     hphi[c] = rhs;
+    // psi, r = sqrt(q) of phi_new for the interface sweep (same formulas as k_iface_psi)
+    const double ph = fz_clip01(fn);
+    const double q = (ph + P.delta) / (1.0 - ph + P.delta);
+    psi[c] = P.eps * log(q);
+    rr[c] = sqrt(q);
 }
 
 // ---------------------------------------------------------------- S2b: temperature transport (N14)

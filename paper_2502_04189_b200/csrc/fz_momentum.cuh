@@ -189,29 +189,28 @@ k_momentum(FzP P, FzMomArgs A)
 
 // =====================================================================================
 // 2.5-D marching variant (the one used when nx >= 32 and ny >= 8).  A CTA owns an x-y tile of
-// MTX x MTY cells and marches over a chunk of z planes.  Every staged field keeps a ring of four
-// planes (tile + halo 1) in shared memory, so each plane is read from HBM once per chunk, all
-// 60-odd neighbour reads of the stencil are shared-memory reads, and the global loads of plane
-// k+2 are issued before the arithmetic of plane k (software prefetch through registers): DRAM
-// latency is hidden by the pipeline rather than by occupancy.  One barrier per plane: with four
-// slots the plane written at step k (k+1) is never one that a lagging warp may still read
-// (k-2 .. k).  Wall ghosts (no-slip: -u, -v; impermeable: w = 0, R_z = 0; mirror: phi, kappa,
-// p_hat; Dirichlet: 2 T_wall - T) are applied when a ghost plane is written into the ring.
+// MTX x MTY cells and marches over a chunk of z planes.  Every staged field keeps a ring of five
+// planes (tile + halo 2 in x, 1 in y) in shared memory, filled by 16-byte cp.async copies (LDGSTS)
+// issued two planes ahead of their use: each plane is read from HBM once per chunk, all 60-odd
+// neighbour reads of the stencil are shared-memory reads, and no register is tied up by a load in
+// flight -- DRAM latency is hidden by the pipeline rather than by occupancy.  One barrier per
+// plane.  Wall ghosts (no-slip: -u, -v; impermeable: w = 0, R_z = 0; mirror: phi, kappa, p_hat)
+// are applied when a ghost plane is READ: the ring holds the mirrored source plane unchanged.
 #define MTX 32
 #define MTY 8
-#define MPW (MTX + 2)
+#define MPW (MTX + 4)
 #define MPH (MTY + 2)
 #define MPS (MPW * MPH)
-#define MRING 4
-#define MHALO (MPS - MTX * MTY)
+#define MRING 5
+#define MCHUNKS (MPS / 2)
 
 template <bool VARRHO, bool HEAT>
 struct FzMomFields {
     static constexpr int U = 0, V = 1, W = 2, PHI = 3, KAP = 4;
     static constexpr int T = 5;                        // valid if HEAT
     static constexpr int RX = 5 + (HEAT ? 1 : 0);      // valid if VARRHO
-    static constexpr int RY = RX + 1, RZ = RX + 2, PH = RX + 3;
-    static constexpr int NF = 5 + (HEAT ? 1 : 0) + (VARRHO ? 4 : 0);
+    static constexpr int RY = RX + 1, RZ = RX + 2, PN = RX + 3, PO = RX + 4;   // p and p_prev
+    static constexpr int NF = 5 + (HEAT ? 1 : 0) + (VARRHO ? 5 : 0);
 };
 
 template <bool VARRHO, bool VARMU, bool HEAT>
@@ -220,98 +219,73 @@ k_momentum_march(FzP P, FzMomArgs A, int KC)
 {
     using F = FzMomFields<VARRHO, HEAT>;
     constexpr int NF = F::NF;
-    extern __shared__ double smm[];  // [NF][MRING][MPS]
+    extern __shared__ __align__(16) double smm[];  // [NF][MRING][MPS]
     const int tx = threadIdx.x, ty = threadIdx.y, t = ty * MTX + tx;
     const int i0 = blockIdx.x * MTX, j0 = blockIdx.y * MTY;
     const int i = i0 + tx, j = j0 + ty;
     const int k0 = blockIdx.z * KC, k1 = min(k0 + KC, P.nz);
-    const int cidx = (ty + 1) * MPW + (tx + 1);
-    // this thread's halo point (threads 0..MHALO-1): top row, bottom row, left column, right column
-    int hx = 0, hy = 0;
-    if (t < MPW) { hx = t - 1; hy = -1; }
-    else if (t < 2 * MPW) { hx = t - MPW - 1; hy = MTY; }
-    else if (t < 2 * MPW + MTY) { hx = -1; hy = t - 2 * MPW; }
-    else { hx = MTX; hy = t - 2 * MPW - MTY; }
-    const bool has_halo = t < MHALO;
-    const int hidx = (hy + 1) * MPW + (hx + 1);
+    const int cidx = (ty + 1) * MPW + (tx + 2);
     const long long goff_c = i + (long long)P.nx * j;
-    const long long goff_h = ((i0 + hx + P.nx) & (P.nx - 1)) + (long long)P.nx * ((j0 + hy + P.ny) & (P.ny - 1));
+    // staging map: thread t < MCHUNKS copies 16-byte chunk t of the staged rectangle of every field
+    const bool loader = t < MCHUNKS;
+    const int lrow = t / (MPW / 2), lcp = t - lrow * (MPW / 2);
+    const long long goff_l = ((i0 - 2 + 2 * lcp + P.nx) & (P.nx - 1)) +
+                             (long long)P.nx * ((j0 - 1 + lrow + P.ny) & (P.ny - 1));
+    const int soff = lrow * MPW + 2 * lcp;
 
     const double *src[NF];
     src[F::U] = A.u; src[F::V] = A.v; src[F::W] = A.w; src[F::PHI] = A.phi; src[F::KAP] = A.kappa;
     if (HEAT) src[F::T] = A.T;
-    if (VARRHO) { src[F::RX] = A.rnx; src[F::RY] = A.rny; src[F::RZ] = A.rnz; src[F::PH] = A.p; }
+    if (VARRHO) { src[F::RX] = A.rnx; src[F::RY] = A.rny; src[F::RZ] = A.rnz; src[F::PN] = A.p; src[F::PO] = A.pp; }
 
-    double rc[NF], rh[NF];
-    // fetch plane kk (k0-1 .. k1) of every staged field into registers, ghost rules applied
-    auto fetch = [&](int kk) {
-        int sp = kk;
-        int ghost = 0;  // -1 bottom wall ghost, +1 top wall ghost
-        if (P.z_wall) {
-            if (kk < 0) { sp = 0; ghost = -1; }
-            else if (kk >= P.nz) { sp = P.nz - 1; ghost = 1; }
-        } else {
-            sp = kk < 0 ? kk + P.nz : (kk >= P.nz ? kk - P.nz : kk);
-        }
-        const long long pc = (long long)sp * P.sxy + goff_c, ph = (long long)sp * P.sxy + goff_h;
+    // copy plane kk (k0-1 .. k1; ghosts: periodic wrap or wall mirror) of every field into ring slot kk mod 5
+    auto issue = [&](int kk) {
+        if (loader && kk <= k1) {
+            int sp = kk;
+            if (P.z_wall) sp = kk < 0 ? 0 : (kk >= P.nz ? P.nz - 1 : kk);
+            else sp = kk < 0 ? kk + P.nz : (kk >= P.nz ? kk - P.nz : kk);
+            const long long g = (long long)sp * P.sxy + goff_l;
+            const int o = ((kk + MRING) % MRING) * MPS + soff;
 #pragma unroll
-        for (int f = 0; f < NF; ++f) {
-            double a = src[f][pc];
-            double b = has_halo ? src[f][ph] : 0.0;
-            if (VARRHO && f == F::PH) {  // p_hat = 2 p - p_prev (N7)
-                a = 2.0 * a - A.pp[pc];
-                if (has_halo) b = 2.0 * b - A.pp[ph];
-            }
-            if (ghost != 0) {
-                if (f == F::U || f == F::V) { a = -a; b = -b; }
-                else if (f == F::W || (VARRHO && f == F::RZ)) { a = 0.0; b = 0.0; }
-                else if (HEAT && f == F::T) {
-                    const double tw = ghost < 0 ? P.t_bot : P.t_top;
-                    a = 2.0 * tw - a; b = 2.0 * tw - b;
-                }
-            }
-            rc[f] = a; rh[f] = b;
+            for (int f = 0; f < NF; ++f) fz_cp_async16(smm + f * (MRING * MPS) + o, src[f] + g);
         }
     };
-    auto stash = [&](int kk) {
-        const int slot = (kk + MRING) & (MRING - 1);
-#pragma unroll
-        for (int f = 0; f < NF; ++f) {
-            double *pl = smm + (f * MRING + slot) * MPS;
-            pl[cidx] = rc[f];
-            if (has_halo) pl[hidx] = rh[f];
-        }
-    };
-
-    fetch(k0 - 1); stash(k0 - 1);
-    fetch(k0); stash(k0);
-    fetch(k0 + 1);
+    issue(k0 - 1); issue(k0); fz_cp_async_commit();
+    issue(k0 + 1); fz_cp_async_commit();
+    issue(k0 + 2); fz_cp_async_commit();
 
     const double dx = P.idx, dy = P.idy;
     const double dmu = P.mu1 - P.mu2;
     const double ir0 = 1.0 / P.rho0;
     const double Gam = A.scal[1];
 
+    int sl = (k0 - 1 + MRING) % MRING;   // ring slot of plane k-1, advanced incrementally
+    int om, o0 = sl * MPS + cidx, op = ((sl + 1) % MRING) * MPS + cidx;
+    sl = (sl + 1) % MRING;
     for (int k = k0; k < k1; ++k) {
-        stash(k + 1);
+        fz_cp_async_wait<1>();
         __syncthreads();
-        if (k + 2 <= k1) fetch(k + 2);
+        issue(k + 3);
+        fz_cp_async_commit();
+        sl = (sl + 1 == MRING) ? 0 : sl + 1;
+        om = o0; o0 = op; op = sl * MPS + cidx;   // planes k-1, k, k+1
         const long long c = (long long)k * P.sxy + goff_c;
         const double hu_old = A.hu[c], hv_old = A.hv[c], hw_old = A.hw[c];
-        const int om = ((k - 1 + MRING) & (MRING - 1)) * MPS + cidx, o0 = (k & (MRING - 1)) * MPS + cidx,
-                  op = ((k + 1) & (MRING - 1)) * MPS + cidx;
+        // ghost rules at the walls: planes k-1 / k+1 hold the mirrored interior plane
+        const bool gm = P.z_wall && k == 0, gp = P.z_wall && k == P.nz - 1;
+        const double sgm = gm ? -1.0 : 1.0, sgp = gp ? -1.0 : 1.0, wm = gm ? 0.0 : 1.0;
         // S(f, di, dj, plane offset) -- shared-memory neighbour read
-#define S_(f, di, dj, o) smm[(f) * (MRING * MPS) + (o) + (dj) * MPW + (di)]
+#define S_(f, di, dj, o) smm[(f) * (MRING * MPS) + (o) + (dj) * MPW + (di)]   // o includes cidx
         const double izf = P.idzf[k], izc = P.idzc[k], izcm = P.idzc[k - 1];
         const double u000 = S_(F::U, 0, 0, o0), up00 = S_(F::U, 1, 0, o0), um00 = S_(F::U, -1, 0, o0);
         const double u0p0 = S_(F::U, 0, 1, o0), u0m0 = S_(F::U, 0, -1, o0), ump0 = S_(F::U, -1, 1, o0);
-        const double u00p = S_(F::U, 0, 0, op), u00m = S_(F::U, 0, 0, om), um0p = S_(F::U, -1, 0, op);
+        const double u00p = sgp * S_(F::U, 0, 0, op), u00m = sgm * S_(F::U, 0, 0, om), um0p = sgp * S_(F::U, -1, 0, op);
         const double v000 = S_(F::V, 0, 0, o0), vp00 = S_(F::V, 1, 0, o0), vm00 = S_(F::V, -1, 0, o0);
         const double v0p0 = S_(F::V, 0, 1, o0), v0m0 = S_(F::V, 0, -1, o0), vpm0 = S_(F::V, 1, -1, o0);
-        const double v00p = S_(F::V, 0, 0, op), v00m = S_(F::V, 0, 0, om), v0mp = S_(F::V, 0, -1, op);
+        const double v00p = sgp * S_(F::V, 0, 0, op), v00m = sgm * S_(F::V, 0, 0, om), v0mp = sgp * S_(F::V, 0, -1, op);
         const double w000 = S_(F::W, 0, 0, o0), wp00 = S_(F::W, 1, 0, o0), wm00 = S_(F::W, -1, 0, o0);
         const double w0p0 = S_(F::W, 0, 1, o0), w0m0 = S_(F::W, 0, -1, o0);
-        const double w00m = S_(F::W, 0, 0, om), wp0m = S_(F::W, 1, 0, om), w0pm = S_(F::W, 0, 1, om);
+        const double w00m = wm * S_(F::W, 0, 0, om), wp0m = wm * S_(F::W, 1, 0, om), w0pm = wm * S_(F::W, 0, 1, om);
         const double f000 = S_(F::PHI, 0, 0, o0), fp00 = S_(F::PHI, 1, 0, o0), f0p0 = S_(F::PHI, 0, 1, o0),
                      f00p = S_(F::PHI, 0, 0, op);
         double m000, mp00, mm00, m0p0, m0m0, m00p, m00m, mpp0, mpm0, mmp0, mp0p, mp0m, mm0p, m0pp, m0pm, m0mp;
@@ -335,8 +309,11 @@ k_momentum_march(FzP P, FzMomArgs A, int KC)
             irx = 1.0 / (0.5 * (r000 + P.rho2 + P.drho * fz_clip01(fp00)));
             iry = 1.0 / (0.5 * (r000 + P.rho2 + P.drho * fz_clip01(f0p0)));
             irz = 1.0 / (0.5 * (r000 + P.rho2 + P.drho * fz_clip01(f00p)));
-            ph000 = S_(F::PH, 0, 0, o0); php00 = S_(F::PH, 1, 0, o0); ph0p0 = S_(F::PH, 0, 1, o0);
-            ph00p = S_(F::PH, 0, 0, op);
+            // p_hat = 2 p - p_prev (N7)
+#define PH_(di, dj, o) (2.0 * S_(F::PN, di, dj, o) - S_(F::PO, di, dj, o))
+            ph000 = PH_(0, 0, o0); php00 = PH_(1, 0, o0); ph0p0 = PH_(0, 1, o0);
+            ph00p = PH_(0, 0, op);
+#undef PH_
         }
         double T000 = 0;
         if (HEAT) T000 = S_(F::T, 0, 0, o0);
@@ -358,7 +335,7 @@ k_momentum_march(FzP P, FzMomArgs A, int KC)
             double M = 0.0;
             if (VARRHO) {
                 const double Rty = 0.25 * (S_(F::RY, 0, 0, o0) + S_(F::RY, 1, 0, o0) + S_(F::RY, 0, -1, o0) + S_(F::RY, 1, -1, o0));
-                const double Rtz = 0.25 * (S_(F::RZ, 0, 0, o0) + S_(F::RZ, 1, 0, o0) + S_(F::RZ, 0, 0, om) + S_(F::RZ, 1, 0, om));
+                const double Rtz = 0.25 * (S_(F::RZ, 0, 0, o0) + S_(F::RZ, 1, 0, o0) + wm * (S_(F::RZ, 0, 0, om) + S_(F::RZ, 1, 0, om)));
                 M = P.drho * Gam * (S_(F::RX, 0, 0, o0) * (up00 - um00) * (0.5 * dx) + Rty * (u0p0 - u0m0) * (0.5 * dy) +
                                     Rtz * (u00p - u00m) * P.igz[k]);
             }
@@ -388,7 +365,7 @@ k_momentum_march(FzP P, FzMomArgs A, int KC)
             double M = 0.0;
             if (VARRHO) {
                 const double Rtx = 0.25 * (S_(F::RX, 0, 0, o0) + S_(F::RX, 0, 1, o0) + S_(F::RX, -1, 0, o0) + S_(F::RX, -1, 1, o0));
-                const double Rtz = 0.25 * (S_(F::RZ, 0, 0, o0) + S_(F::RZ, 0, 1, o0) + S_(F::RZ, 0, 0, om) + S_(F::RZ, 0, 1, om));
+                const double Rtz = 0.25 * (S_(F::RZ, 0, 0, o0) + S_(F::RZ, 0, 1, o0) + wm * (S_(F::RZ, 0, 0, om) + S_(F::RZ, 0, 1, om)));
                 M = P.drho * Gam * (S_(F::RY, 0, 0, o0) * (v0p0 - v0m0) * (0.5 * dy) + Rtx * (vp00 - vm00) * (0.5 * dx) +
                                     Rtz * (v00p - v00m) * P.igz[k]);
             }

@@ -43,8 +43,10 @@ def algorithmic_bytes_per_cell(cfg):
         "k_phi_update": 80.0,                                   # r phi,u,v,w,hphi,divRn  w phi,hphi,psi,r
         "k_iface_march": 40.0 + (24.0 if varrho else 0.0),      # r psi,r,phi  w kappa,divRn (+Rn x3)
         "k_momentum": 112.0 + (40.0 if varrho else 0.0) + (8.0 if heat else 0.0),
-        "k_fftx_fwd": 24.0 + spec, "k_ffty_fwd": 2 * spec, "k_tridiag": 2 * spec,
-        "k_ffty_inv": 2 * spec, "k_fftx_inv": spec + 8.0, "k_correct": 56.0,
+        "k_fftx_fwd": 24.0 + spec,
+        # fused FFT_y + z-elimination: r spec, INV (half a complex), w spec; backward also E if z is periodic
+        "k_spec_fwd": 2.5 * spec, "k_spec_bwd": (3.0 if not cfg["z_wall"] else 2.5) * spec,
+        "k_fftx_inv": spec + 8.0, "k_correct": 56.0,
     }
     if heat:
         b["k_temp_update"] = 64.0

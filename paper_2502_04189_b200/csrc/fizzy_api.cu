@@ -14,7 +14,7 @@
 #include "fz_iface.cuh"
 #include "fz_momentum.cuh"
 #include "fz_stencil.cuh"
-#include "fz_tridiag.cuh"
+#include "fz_spectral.cuh"
 
 namespace {
 
@@ -37,10 +37,10 @@ struct Carver {  // hands out 256-byte aligned pieces of the workspace (or just 
 }  // namespace
 
 enum FzKernelId { FZK_LATCH, FZK_PHI, FZK_IMARCH, FZK_IPSI, FZK_INHAT, FZK_IFLUX, FZK_TEMP, FZK_MOM, FZK_FFTX_FWD,
-                  FZK_FFTY_FWD, FZK_TRI, FZK_GAUGE, FZK_FFTY_INV, FZK_FFTX_INV, FZK_CORRECT, FZK_OTHER, FZK_COUNT };
+                  FZK_SPEC_FWD, FZK_SPEC_BWD, FZK_FFTX_INV, FZK_CORRECT, FZK_OTHER, FZK_COUNT };
 static const char *const FZK_NAME[FZK_COUNT] = {
     "k_latch_gamma", "k_phi_update", "k_iface_march", "k_iface_psi", "k_iface_nhat", "k_iface_flux", "k_temp_update", "k_momentum",
-    "k_fftx_fwd", "k_ffty_fwd", "k_tridiag", "k_gauge", "k_ffty_inv", "k_fftx_inv", "k_correct", "other"};
+    "k_fftx_fwd", "k_spec_fwd", "k_spec_bwd", "k_fftx_inv", "k_correct", "other"};
 
 struct FzTimed { int id; cudaEvent_t e0, e1; };
 
@@ -54,8 +54,8 @@ struct fizzy_ctx {
     long long t_n[FZK_COUNT] = {0};
     cudaStream_t stream;
     bool varrho, varmu, heat, cyclic;
-    int log2nx, log2ny, Sx, Sy;
-    size_t smem_x, smem_y;
+    int log2nx, log2ny, Sx;
+    size_t smem_x, smem_yf, smem_yb;
     long long N, M;
     // fields
     double *u, *v, *w, *us, *vs, *ws, *hu, *hv, *hw;
@@ -118,8 +118,8 @@ size_t layout(fizzy_ctx *c, void *base, const fizzy_grid *g, const fizzy_bc *bc,
     if (pr->heat) { x->T = cv.dbl(N); x->Tn = cv.dbl(N); x->hT = cv.dbl(N); }
     x->spec = static_cast<double2 *>(cv.take(M * g->nz * sizeof(double2)));
     x->tri.inv = cv.dbl(M * g->nz);
-    x->tri.e = x->tri.f = x->tri.ginv = nullptr;
-    if (cyclic) { x->tri.e = cv.dbl(M * g->nz); x->tri.f = cv.dbl(M * g->nz); x->tri.ginv = cv.dbl(M); }
+    x->tri.e = x->tri.ginv = nullptr;
+    if (cyclic) { x->tri.e = cv.dbl(M * g->nz); x->tri.ginv = cv.dbl(M); }
     for (int q = 0; q < 5; ++q) { double *t = cv.dbl(g->nz + 2 * FZ_H); if (ztab) ztab[q] = t; }
     for (int q = 0; q < 2; ++q) { double *t = cv.dbl(g->nz); if (acoef) acoef[q] = t; }
     { double *t = cv.dbl(nxh); if (lam) lam[0] = t; t = cv.dbl(g->ny); if (lam) lam[1] = t; }
@@ -239,9 +239,9 @@ extern "C" fizzy_status fizzy_create(const fizzy_grid *grid, const fizzy_bc *bc,
     // S lines side by side per CTA: 256 threads for n <= 512, 512 threads for n = 1024
     auto pick_s = [](int n) { return n >= 1024 ? 4 : (n >= 256 ? 2048 / n : (n >= 32 ? 8 : 256 / n)); };
     c->Sx = pick_s(nx);
-    c->Sy = pick_s(ny);
     c->smem_x = (size_t)nx * (c->Sx + 1) * sizeof(double2);
-    c->smem_y = (size_t)ny * (c->Sy + 1) * sizeof(double2);
+    c->smem_yf = fz_spec_smem(ny, false);
+    c->smem_yb = fz_spec_smem(ny, c->cyclic);
 
     // ---- 1-D z metrics with ghosts (walls mirror, periodic wraps), N10: centres = face midpoints
     const int nzt = nz + 2 * FZ_H;
@@ -282,7 +282,7 @@ extern "C" fizzy_status fizzy_create(const fizzy_grid *grid, const fizzy_bc *bc,
     FZ_CUDA(cudaStreamSynchronize(c->stream));  // the host vectors go out of scope below
 
     c->tri.a = acoef[0]; c->tri.c = acoef[1]; c->tri.lamx = lam[0]; c->tri.lamy = lam[1];
-    c->tri.M = c->M; c->tri.cyclic = c->cyclic ? 1 : 0;
+    c->tri.cyclic = c->cyclic ? 1 : 0;
     FZ_TB(FZK_OTHER);
     k_tri_tables<<<(unsigned)((c->M + 127) / 128), 128, 0, c->stream>>>(P, c->tri);
     FZ_LAUNCHED(FZK_OTHER);
@@ -293,8 +293,10 @@ extern "C" fizzy_status fizzy_create(const fizzy_grid *grid, const fizzy_bc *bc,
     FZ_CUDA(cudaFuncSetAttribute(k_fftx_fwd<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_x));
     FZ_CUDA(cudaFuncSetAttribute(k_fftx_fwd<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_x));
     FZ_CUDA(cudaFuncSetAttribute(k_fftx_inv, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_x));
-    FZ_CUDA(cudaFuncSetAttribute(k_ffty<-1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_y));
-    FZ_CUDA(cudaFuncSetAttribute(k_ffty<+1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_y));
+    FZ_CUDA(cudaFuncSetAttribute(k_spec_fwd<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_yf));
+    FZ_CUDA(cudaFuncSetAttribute(k_spec_fwd<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_yf));
+    FZ_CUDA(cudaFuncSetAttribute(k_spec_bwd<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_yb));
+    FZ_CUDA(cudaFuncSetAttribute(k_spec_bwd<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_yb));
     return FIZZY_OK;
 }
 
@@ -395,31 +397,26 @@ fizzy_status run_interface(fizzy_ctx *c, bool with_psi)
     return FIZZY_OK;
 }
 
-// spectral part of S4 on c->spec (forward x-transform already done): y-FFT, z-solve, gauge, inverse
+// spectral part of S4 on c->spec (forward x-transform already done): fused FFT_y + z elimination,
+// back substitution + inverse FFT_y (gauge mean -> scal[2]), inverse x-transform (- gauge shift)
 fizzy_status run_spectral_solve(fizzy_ctx *c, double *dst)
 {
     const FzP &P = c->P;
-    const dim3 gy((P.nxh + c->Sy - 1) / c->Sy, P.nz);
-    const int ty = c->Sy * P.ny / 8, tx = c->Sx * P.nx / 8;
-    FZ_TB(FZK_FFTY_FWD);
-    k_ffty<-1><<<gy, ty, c->smem_y, c->stream>>>(P, c->spec, c->twy, c->log2ny, c->Sy);
-    FZ_LAUNCHED(FZK_FFTY_FWD);
-    const unsigned gt = (unsigned)((c->M + 127) / 128);
-    FZ_TB(FZK_TRI);
-    if (c->cyclic) k_tridiag<true><<<gt, 128, 0, c->stream>>>(P, c->tri, c->spec);
-    else k_tridiag<false><<<gt, 128, 0, c->stream>>>(P, c->tri, c->spec);
-    FZ_LAUNCHED(FZK_TRI);
-    FZ_TB(FZK_GAUGE);
-    k_gauge<<<1, 256, 0, c->stream>>>(P, c->spec, c->M);
-    FZ_LAUNCHED(FZK_GAUGE);
-    FZ_TB(FZK_FFTY_INV);
-    k_ffty<+1><<<gy, ty, c->smem_y, c->stream>>>(P, c->spec, c->twy, c->log2ny, c->Sy);
-    FZ_LAUNCHED(FZK_FFTY_INV);
+    const int ty = P.ny / 8;
+    FZ_TB(FZK_SPEC_FWD);
+    if (c->cyclic) k_spec_fwd<true><<<P.nxh, ty, c->smem_yf, c->stream>>>(P, c->tri, c->spec, c->twy, c->log2ny);
+    else k_spec_fwd<false><<<P.nxh, ty, c->smem_yf, c->stream>>>(P, c->tri, c->spec, c->twy, c->log2ny);
+    FZ_LAUNCHED(FZK_SPEC_FWD);
+    FZ_TB(FZK_SPEC_BWD);
+    if (c->cyclic) k_spec_bwd<true><<<P.nxh, ty, c->smem_yb, c->stream>>>(P, c->tri, c->spec, c->twy, c->log2ny, c->scal);
+    else k_spec_bwd<false><<<P.nxh, ty, c->smem_yb, c->stream>>>(P, c->tri, c->spec, c->twy, c->log2ny, c->scal);
+    FZ_LAUNCHED(FZK_SPEC_BWD);
     const long long nlines = (long long)P.ny * P.nz;
     const unsigned gx = (unsigned)((nlines + 2 * c->Sx - 1) / (2 * c->Sx));
+    const int tx = c->Sx * P.nx / 8;
     FZ_TB(FZK_FFTX_INV);
     k_fftx_inv<<<gx, tx, c->smem_x, c->stream>>>(P, c->spec, dst, 1.0 / ((double)P.nx * (double)P.ny), c->twx,
-                                                 c->log2nx, c->Sx);
+                                                 c->log2nx, c->Sx, c->scal);
     FZ_LAUNCHED(FZK_FFTX_INV);
     return FIZZY_OK;
 }

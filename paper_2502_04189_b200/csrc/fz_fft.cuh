@@ -56,10 +56,14 @@ __device__ __forceinline__ void fz_dft8(double2 (&v)[8])
 
 // One Stockham pass of radix R over the S side-by-side FFTs held in sm (in place: all loads,
 // barrier, all stores, barrier).  jt in [0, n/8) is this thread's index within its FFT.
-template <int R, int SGN>
+// PAD = true: a single line per CTA stored as sm[i + (i >> 3)] (one 16-byte pad per 8 elements),
+// which makes every butterfly load/store of the radix-8 passes conflict free without side-by-side
+// lines (slot and LP are ignored).
+template <int R, int SGN, bool PAD = false>
 __device__ __forceinline__ void fz_fft_pass(double2 *sm, const double2 *__restrict__ tw, int n, int Ns,
                                             int jt, int slot, int LP)
 {
+#define FZ_SMI(i_) (PAD ? ((i_) + ((i_) >> 3)) : ((i_) * LP + slot))
     constexpr int NB = 8 / R;  // butterflies per thread
     const int T = n / R;       // butterflies per FFT
     const int T8 = n >> 3;
@@ -68,7 +72,7 @@ __device__ __forceinline__ void fz_fft_pass(double2 *sm, const double2 *__restri
     for (int b = 0; b < NB; ++b) {
         const int j = jt + b * T8;
 #pragma unroll
-        for (int r = 0; r < R; ++r) v[b][r] = sm[(j + r * T) * LP + slot];
+        for (int r = 0; r < R; ++r) v[b][r] = sm[FZ_SMI(j + r * T)];
     }
     __syncthreads();
 #pragma unroll
@@ -93,31 +97,33 @@ __device__ __forceinline__ void fz_fft_pass(double2 *sm, const double2 *__restri
         }
         const int base = (j - kk) * R + kk;
 #pragma unroll
-        for (int r = 0; r < R; ++r) sm[(base + r * Ns) * LP + slot] = v[b][r];
+        for (int r = 0; r < R; ++r) sm[FZ_SMI(base + r * Ns)] = v[b][r];
     }
     __syncthreads();
+#undef FZ_SMI
 }
 
 // Full FFT of the S lines in sm.  Data must be in sm and visible (barrier done by the caller).
-template <int SGN>
+template <int SGN, bool PAD = false>
 __device__ __forceinline__ void fz_fft_tile(double2 *sm, const double2 *__restrict__ tw, int n, int log2n,
                                             int jt, int slot, int LP)
 {
     int Ns = 1;
     const int n8 = log2n / 3;
     for (int q = 0; q < n8; ++q) {
-        fz_fft_pass<8, SGN>(sm, tw, n, Ns, jt, slot, LP);
+        fz_fft_pass<8, SGN, PAD>(sm, tw, n, Ns, jt, slot, LP);
         Ns <<= 3;
     }
     const int rem = log2n - 3 * n8;
-    if (rem == 2) fz_fft_pass<4, SGN>(sm, tw, n, Ns, jt, slot, LP);
-    else if (rem == 1) fz_fft_pass<2, SGN>(sm, tw, n, Ns, jt, slot, LP);
+    if (rem == 2) fz_fft_pass<4, SGN, PAD>(sm, tw, n, Ns, jt, slot, LP);
+    else if (rem == 1) fz_fft_pass<2, SGN, PAD>(sm, tw, n, Ns, jt, slot, LP);
 }
 
 // ---------------------------------------------------------------- FFT along x, forward
 // Lines are (j,k) pairs flattened as L = j + ny*k; a CTA takes 2S consecutive lines, two real
 // lines per complex FFT (a + i b), and writes nxh = nx/2+1 modes per line:
-//   spec[L*nxh + l].   A_l = (Z_l + conj Z_{n-l})/2,  B_l = (Z_l - conj Z_{n-l})/(2i).
+//   spec[(k*nxh + l)*ny + j]   (y lines contiguous, see fz_spectral.cuh).
+//   A_l = (Z_l + conj Z_{n-l})/2,  B_l = (Z_l - conj Z_{n-l})/(2i).
 // DIV = true: the real input is the Poisson right-hand side assembled on the fly,
 //   b = coef * D(u**)  (BASELINE.json:5(iv) with the p_hat term folded into u**, D2);
 // DIV = false: the real input is read from `src` (fizzy_poisson_solve).
@@ -156,10 +162,10 @@ __global__ void __launch_bounds__(512, 2) k_fftx_fwd(FzP P, const double *__rest
     __syncthreads();
     const int slot = threadIdx.x % S, jt = threadIdx.x / S;
     fz_fft_tile<-1>(sm, tw, n, log2n, jt, slot, LP);
-    // untangle and store
-    const int nxh = P.nxh;
+    // untangle and store: spec[(k*nxh + l)*ny + j], j fastest -> 2S consecutive lines give 32*S-byte runs
+    const int nxh = P.nxh, lgy = __ffs(P.ny) - 1;
     for (int e = threadIdx.x; e < 2 * S * nxh; e += nth) {
-        const int ln = e / nxh, l = e - ln * nxh;
+        const int l = e / (2 * S), ln = e - l * (2 * S);
         const long long L = L0 + ln;
         if (L >= nlines) continue;
         const int sl = ln >> 1;
@@ -168,27 +174,30 @@ __global__ void __launch_bounds__(512, 2) k_fftx_fwd(FzP P, const double *__rest
         double2 o;
         if (ln & 1) o = make_double2(0.5 * (z1.y + z2.y), -0.5 * (z1.x - z2.x));  // B_l
         else o = make_double2(0.5 * (z1.x + z2.x), 0.5 * (z1.y - z2.y));          // A_l
-        spec[L * nxh + l] = o;
+        const long long k = L >> lgy, j = L & (P.ny - 1);
+        spec[(k * nxh + l) * P.ny + j] = o;
     }
 }
 
 // ---------------------------------------------------------------- FFT along x, backward (c2r)
-// Z_l = A_l + i B_l, Z_{n-l} = conj(A_l) + i conj(B_l); out = Re/Im of the inverse transform * scale
+// Z_l = A_l + i B_l, Z_{n-l} = conj(A_l) + i conj(B_l); out = Re/Im of the inverse transform * scale - gauge shift
 __global__ void __launch_bounds__(512, 2) k_fftx_inv(FzP P, const double2 *__restrict__ spec, double *__restrict__ dst, double scale,
-                           const double2 *__restrict__ tw, int log2n, int S)
+                           const double2 *__restrict__ tw, int log2n, int S, const double *__restrict__ scal)
 {
     extern __shared__ double2 sm[];
     const int n = P.nx, LP = S + 1, nxh = P.nxh;
     const int nth = blockDim.x;
     const long long nlines = (long long)P.ny * P.nz;
     const long long L0 = (long long)blockIdx.x * 2 * S;
+    const int lgy = __ffs(P.ny) - 1;
+    const double shift = scal[2] * scale;   // gauge (N17): mean of mode (0,0), from k_spec_bwd
     // pairs of lines: slot sl holds lines 2 sl (A) and 2 sl + 1 (B)
     for (int e = threadIdx.x; e < S * nxh; e += nth) {
-        const int sl = e / nxh, l = e - sl * nxh;
+        const int l = e / S, sl = e - l * S;
         const long long LA = L0 + 2 * sl, LB = LA + 1;
         double2 a = make_double2(0, 0), b = make_double2(0, 0);
-        if (LA < nlines) a = spec[LA * nxh + l];
-        if (LB < nlines) b = spec[LB * nxh + l];
+        if (LA < nlines) { const long long k = LA >> lgy, j = LA & (P.ny - 1); a = spec[(k * nxh + l) * P.ny + j]; }
+        if (LB < nlines) { const long long k = LB >> lgy, j = LB & (P.ny - 1); b = spec[(k * nxh + l) * P.ny + j]; }
         if (l == 0 || l == n / 2) {
             sm[l * LP + sl] = make_double2(a.x, b.x);
         } else {
@@ -204,31 +213,7 @@ __global__ void __launch_bounds__(512, 2) k_fftx_inv(FzP P, const double2 *__res
         const long long L = L0 + ln;
         if (L >= nlines) continue;
         const double *d = reinterpret_cast<const double *>(&sm[i * LP + (ln >> 1)]);
-        dst[L * n + i] = d[ln & 1] * scale;
+        dst[L * n + i] = d[ln & 1] * scale - shift;
     }
 }
 
-// ---------------------------------------------------------------- FFT along y (complex, in place)
-// CTA = (block of S consecutive l, plane k); element m of slot s is spec[(k*ny + m)*nxh + l0 + s].
-template <int SGN>
-__global__ void __launch_bounds__(512, 2) k_ffty(FzP P, double2 *__restrict__ spec, const double2 *__restrict__ tw, int log2n, int S)
-{
-    extern __shared__ double2 sm[];
-    const int n = P.ny, LP = S + 1, nxh = P.nxh;
-    const int nth = blockDim.x;
-    const int l0 = blockIdx.x * S;
-    const long long base = (long long)blockIdx.y * n * nxh;
-    for (int e = threadIdx.x; e < S * n; e += nth) {
-        const int m = e / S, s = e - m * S;
-        double2 val = make_double2(0, 0);
-        if (l0 + s < nxh) val = spec[base + (long long)m * nxh + l0 + s];
-        sm[m * LP + s] = val;
-    }
-    __syncthreads();
-    const int slot = threadIdx.x % S, jt = threadIdx.x / S;
-    fz_fft_tile<SGN>(sm, tw, n, log2n, jt, slot, LP);
-    for (int e = threadIdx.x; e < S * n; e += nth) {
-        const int m = e / S, s = e - m * S;
-        if (l0 + s < nxh) spec[base + (long long)m * nxh + l0 + s] = sm[m * LP + s];
-    }
-}

@@ -118,7 +118,7 @@ def test_device_pointers_and_state_errors(fz):
     assert torch.equal(out, dev["phi"])
     n0 = g.fizzy_launch_count()
     g.step(dt)
-    assert g.fizzy_launch_count() - n0 >= 3 * 10
+    assert g.fizzy_launch_count() - n0 >= 3 * 8
     bad = dict(cfg)
     bad["nx"] = 24
     with pytest.raises(fz.FizzyError):

@@ -55,7 +55,7 @@ struct fizzy_ctx {
     cudaStream_t stream;
     bool varrho, varmu, heat, cyclic;
     int log2nx, log2ny, Sx;
-    size_t smem_x, smem_yf, smem_yb;
+    size_t smem_x;
     long long N, M;
     // fields
     double *u, *v, *w, *us, *vs, *ws, *hu, *hv, *hw;
@@ -240,8 +240,6 @@ extern "C" fizzy_status fizzy_create(const fizzy_grid *grid, const fizzy_bc *bc,
     auto pick_s = [](int n) { return n >= 1024 ? 4 : (n >= 256 ? 2048 / n : (n >= 32 ? 8 : 256 / n)); };
     c->Sx = pick_s(nx);
     c->smem_x = (size_t)nx * (c->Sx + 1) * sizeof(double2);
-    c->smem_yf = fz_spec_smem(ny, false);
-    c->smem_yb = fz_spec_smem(ny, c->cyclic);
 
     // ---- 1-D z metrics with ghosts (walls mirror, periodic wraps), N10: centres = face midpoints
     const int nzt = nz + 2 * FZ_H;
@@ -293,10 +291,6 @@ extern "C" fizzy_status fizzy_create(const fizzy_grid *grid, const fizzy_bc *bc,
     FZ_CUDA(cudaFuncSetAttribute(k_fftx_fwd<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_x));
     FZ_CUDA(cudaFuncSetAttribute(k_fftx_fwd<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_x));
     FZ_CUDA(cudaFuncSetAttribute(k_fftx_inv, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_x));
-    FZ_CUDA(cudaFuncSetAttribute(k_spec_fwd<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_yf));
-    FZ_CUDA(cudaFuncSetAttribute(k_spec_fwd<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_yf));
-    FZ_CUDA(cudaFuncSetAttribute(k_spec_bwd<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_yb));
-    FZ_CUDA(cudaFuncSetAttribute(k_spec_bwd<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_yb));
     return FIZZY_OK;
 }
 
@@ -402,14 +396,13 @@ fizzy_status run_interface(fizzy_ctx *c, bool with_psi)
 fizzy_status run_spectral_solve(fizzy_ctx *c, double *dst)
 {
     const FzP &P = c->P;
-    const int ty = P.ny / 8;
     FZ_TB(FZK_SPEC_FWD);
-    if (c->cyclic) k_spec_fwd<true><<<P.nxh, ty, c->smem_yf, c->stream>>>(P, c->tri, c->spec, c->twy, c->log2ny);
-    else k_spec_fwd<false><<<P.nxh, ty, c->smem_yf, c->stream>>>(P, c->tri, c->spec, c->twy, c->log2ny);
+    FZ_CUDA(c->cyclic ? fz_spec_launch<true>(true, c->log2ny, P, c->tri, c->spec, c->twy, c->scal, c->stream)
+                      : fz_spec_launch<false>(true, c->log2ny, P, c->tri, c->spec, c->twy, c->scal, c->stream));
     FZ_LAUNCHED(FZK_SPEC_FWD);
     FZ_TB(FZK_SPEC_BWD);
-    if (c->cyclic) k_spec_bwd<true><<<P.nxh, ty, c->smem_yb, c->stream>>>(P, c->tri, c->spec, c->twy, c->log2ny, c->scal);
-    else k_spec_bwd<false><<<P.nxh, ty, c->smem_yb, c->stream>>>(P, c->tri, c->spec, c->twy, c->log2ny, c->scal);
+    FZ_CUDA(c->cyclic ? fz_spec_launch<true>(false, c->log2ny, P, c->tri, c->spec, c->twy, c->scal, c->stream)
+                      : fz_spec_launch<false>(false, c->log2ny, P, c->tri, c->spec, c->twy, c->scal, c->stream));
     FZ_LAUNCHED(FZK_SPEC_BWD);
     const long long nlines = (long long)P.ny * P.nz;
     const unsigned gx = (unsigned)((nlines + 2 * c->Sx - 1) / (2 * c->Sx));

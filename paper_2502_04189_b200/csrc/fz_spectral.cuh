@@ -26,6 +26,7 @@
 #pragma once
 #include "fz_common.cuh"
 #include "fz_fft.cuh"
+#include "fz_linefft.cuh"
 
 struct FzTri {
     const double *a, *c;        // nz each (1-D)
@@ -83,24 +84,25 @@ __global__ void k_tri_tables(FzP P, FzTri Tt)
     }
 }
 
-// shared memory: twiddles [n] double2 | ring of SPEC_RING padded lines | ring of INV rows (| E rows)
+// shared memory: scratch line | ring of SPEC_RING padded lines | ring of INV rows (| ring of E rows)
 __host__ __device__ inline size_t fz_spec_smem(int n, bool with_e)
 {
-    return (size_t)n * 16 + (size_t)SPEC_RING * ((size_t)SPEC_LINE(n) * 16 + (size_t)n * 8 * (with_e ? 2 : 1));
+    return (size_t)SPEC_LINE(n) * 16 + (size_t)SPEC_RING * ((size_t)SPEC_LINE(n) * 16 + (size_t)n * 8 * (with_e ? 2 : 1));
 }
 
 // ---------------------------------------------------------------- forward: FFT_y + elimination
 // grid = nxh CTAs (one x-mode each), block = ny/8 threads; thread jt owns the systems m = jt + q*ny/8.
-template <bool CYCLIC>
+template <bool CYCLIC, int LOG2N>
 __global__ void __launch_bounds__(128)
-k_spec_fwd(FzP P, FzTri Tt, double2 *__restrict__ spec, const double2 *__restrict__ tw, int log2n)
+k_spec_fwd(FzP P, FzTri Tt, double2 *__restrict__ spec, const double2 *__restrict__ tw)
 {
     extern __shared__ __align__(16) double2 sms[];
-    const int n = P.ny, nt = blockDim.x, jt = threadIdx.x, nz = P.nz;
-    const int LN = SPEC_LINE(n);
-    double2 *tws = sms, *lines = sms + n;
+    constexpr int n = 1 << LOG2N, nt = n / 8, LN = SPEC_LINE(n);
+    const int jt = threadIdx.x, nz = P.nz;
+    double2 *scratch = sms, *lines = sms + LN;
     double *invs = reinterpret_cast<double *>(lines + SPEC_RING * LN);
-    for (int i = jt; i < n; i += nt) tws[i] = tw[i];
+    FzLineFFT<LOG2N, -1> fft;
+    fft.init(tw, jt);
     const long long M = (long long)P.nxh * n, base = (long long)blockIdx.x * n;
     auto issue = [&](int k) {
         if (k < nz) {
@@ -116,7 +118,7 @@ k_spec_fwd(FzP P, FzTri Tt, double2 *__restrict__ spec, const double2 *__restric
         }
     };
     for (int p = 0; p < SPEC_RING - 1; ++p) { issue(p); fz_cp_async_commit(); }
-    double2 dp[8], h[8];
+    double2 dp[8], h[8], v[8];
     double f[8];
     const double c_last = Tt.c[nz - 1], a_last = Tt.a[nz - 1];
 #pragma unroll
@@ -126,8 +128,7 @@ k_spec_fwd(FzP P, FzTri Tt, double2 *__restrict__ spec, const double2 *__restric
         __syncthreads();
         issue(k + SPEC_RING - 1);
         fz_cp_async_commit();
-        double2 *ln = lines + (k & (SPEC_RING - 1)) * LN;
-        fz_fft_tile<-1, true>(ln, tws, n, log2n, jt, 0, 1);
+        fft.smem_to_regs(jt, lines + (k & (SPEC_RING - 1)) * LN, scratch, v);
         const double *iv = invs + (k & (SPEC_RING - 1)) * n;
         double2 *out = spec + (long long)k * M + base;
         const double a = Tt.a[k];
@@ -137,10 +138,9 @@ k_spec_fwd(FzP P, FzTri Tt, double2 *__restrict__ spec, const double2 *__restric
 #pragma unroll
             for (int q = 0; q < 8; ++q) {
                 const int m = jt + q * nt;
-                const double2 d = ln[SPEC_PADI(m)];
                 const double inv = iv[m];
-                dp[q].x = (d.x - a * dp[q].x) * inv;
-                dp[q].y = (d.y - a * dp[q].y) * inv;
+                dp[q].x = (v[q].x - a * dp[q].x) * inv;
+                dp[q].y = (v[q].y - a * dp[q].y) * inv;
                 if (CYCLIC) {
                     const double fk = f[q] + fadd;
                     h[q].x += fk * dp[q].x;
@@ -153,9 +153,8 @@ k_spec_fwd(FzP P, FzTri Tt, double2 *__restrict__ spec, const double2 *__restric
 #pragma unroll
             for (int q = 0; q < 8; ++q) {
                 const int m = jt + q * nt;
-                const double2 d = ln[SPEC_PADI(m)];
                 const double gi = Tt.ginv[base + m];
-                out[m] = make_double2((d.x - h[q].x) * gi, (d.y - h[q].y) * gi);
+                out[m] = make_double2((v[q].x - h[q].x) * gi, (v[q].y - h[q].y) * gi);
             }
         }
     }
@@ -164,18 +163,19 @@ k_spec_fwd(FzP P, FzTri Tt, double2 *__restrict__ spec, const double2 *__restric
 
 // ---------------------------------------------------------------- backward: substitution + inverse FFT_y
 // k descends from nz-1 to 0.  scal[2] receives the dzf-weighted mean of mode (0,0) (gauge, N17).
-template <bool CYCLIC>
+template <bool CYCLIC, int LOG2N>
 __global__ void __launch_bounds__(128)
-k_spec_bwd(FzP P, FzTri Tt, double2 *__restrict__ spec, const double2 *__restrict__ tw, int log2n,
+k_spec_bwd(FzP P, FzTri Tt, double2 *__restrict__ spec, const double2 *__restrict__ tw,
            double *__restrict__ scal)
 {
     extern __shared__ __align__(16) double2 sms[];
-    const int n = P.ny, nt = blockDim.x, jt = threadIdx.x, nz = P.nz;
-    const int LN = SPEC_LINE(n);
-    double2 *tws = sms, *lines = sms + n;
+    constexpr int n = 1 << LOG2N, nt = n / 8, LN = SPEC_LINE(n);
+    const int jt = threadIdx.x, nz = P.nz;
+    double2 *scratch = sms, *lines = sms + LN;
     double *invs = reinterpret_cast<double *>(lines + SPEC_RING * LN);
     double *es = invs + SPEC_RING * n;   // cyclic only
-    for (int i = jt; i < n; i += nt) tws[i] = tw[i];
+    FzLineFFT<LOG2N, +1> fft;
+    fft.init(tw, jt);
     const long long M = (long long)P.nxh * n, base = (long long)blockIdx.x * n;
     auto issue = [&](int s) {   // step s handles plane k = nz-1-s
         if (s < nz) {
@@ -223,15 +223,48 @@ k_spec_bwd(FzP P, FzTri Tt, double2 *__restrict__ spec, const double2 *__restric
                 if (k == nz - 1) X[q] = x;   // row nz-1 holds the separator itself (cc = e = 0)
             }
             xn[q] = x;
-            ln[SPEC_PADI(m)] = x;
         }
         if (gauge) { acc += xn[0].x * P.dzf[k]; vol += P.dzf[k]; }
-        __syncthreads();
-        fz_fft_tile<+1, true>(ln, tws, n, log2n, jt, 0, 1);
+        double2 v[8];
+#pragma unroll
+        for (int q = 0; q < 8; ++q) v[q] = xn[q];
+        const double2 *res = fft.regs_to_smem(jt, ln, scratch, v);
         double2 *out = spec + (long long)k * M + base;
 #pragma unroll
-        for (int q = 0; q < 8; ++q) { const int m = jt + q * nt; out[m] = ln[SPEC_PADI(m)]; }
+        for (int q = 0; q < 8; ++q) { const int m = jt + q * nt; out[m] = res[SPEC_PADI(m)]; }
     }
     if (gauge) scal[2] = acc / vol;
     fz_cp_async_wait<0>();
+}
+
+// ---------------------------------------------------------------- host-side dispatch over log2(ny)
+template <bool CYCLIC, int LOG2N>
+cudaError_t fz_spec_launch_one(bool fwd, const FzP &P, const FzTri &Tt, double2 *spec, const double2 *tw,
+                               double *scal, cudaStream_t st)
+{
+    const int n = 1 << LOG2N;
+    const size_t smem = fz_spec_smem(n, fwd ? false : CYCLIC);
+    cudaError_t e;
+    if (fwd) {
+        e = cudaFuncSetAttribute(k_spec_fwd<CYCLIC, LOG2N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        k_spec_fwd<CYCLIC, LOG2N><<<P.nxh, n / 8, smem, st>>>(P, Tt, spec, tw);
+    } else {
+        e = cudaFuncSetAttribute(k_spec_bwd<CYCLIC, LOG2N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        k_spec_bwd<CYCLIC, LOG2N><<<P.nxh, n / 8, smem, st>>>(P, Tt, spec, tw, scal);
+    }
+    return cudaSuccess;
+}
+
+template <bool CYCLIC>
+cudaError_t fz_spec_launch(bool fwd, int log2n, const FzP &P, const FzTri &Tt, double2 *spec, const double2 *tw,
+                           double *scal, cudaStream_t st)
+{
+    switch (log2n) {
+#define FZ_CASE(L_) case L_: return fz_spec_launch_one<CYCLIC, L_>(fwd, P, Tt, spec, tw, scal, st);
+        FZ_CASE(3) FZ_CASE(4) FZ_CASE(5) FZ_CASE(6) FZ_CASE(7) FZ_CASE(8) FZ_CASE(9) FZ_CASE(10)
+#undef FZ_CASE
+    }
+    return cudaErrorInvalidValue;
 }

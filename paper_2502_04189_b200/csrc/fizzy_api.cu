@@ -10,7 +10,7 @@
 #include <vector>
 
 #include "fz_common.cuh"
-#include "fz_fft.cuh"
+#include "fz_fftx.cuh"
 #include "fz_iface.cuh"
 #include "fz_momentum.cuh"
 #include "fz_stencil.cuh"
@@ -54,8 +54,7 @@ struct fizzy_ctx {
     long long t_n[FZK_COUNT] = {0};
     cudaStream_t stream;
     bool varrho, varmu, heat, cyclic;
-    int log2nx, log2ny, Sx;
-    size_t smem_x;
+    int log2nx, log2ny;
     long long N, M;
     // fields
     double *u, *v, *w, *us, *vs, *ws, *hu, *hv, *hw;
@@ -236,11 +235,6 @@ extern "C" fizzy_status fizzy_create(const fizzy_grid *grid, const fizzy_bc *bc,
     c->N = P.N; c->M = (long long)P.nxh * ny;
     c->varrho = P.rho1 != P.rho2; c->varmu = P.mu1 != P.mu2; c->heat = P.heat != 0; c->cyclic = !bc->z_wall;
     c->log2nx = ilog2(nx); c->log2ny = ilog2(ny);
-    // S lines side by side per CTA: 256 threads for n <= 512, 512 threads for n = 1024
-    auto pick_s = [](int n) { return n >= 1024 ? 4 : (n >= 256 ? 2048 / n : (n >= 32 ? 8 : 256 / n)); };
-    c->Sx = pick_s(nx);
-    c->smem_x = (size_t)nx * (c->Sx + 1) * sizeof(double2);
-
     // ---- 1-D z metrics with ghosts (walls mirror, periodic wraps), N10: centres = face midpoints
     const int nzt = nz + 2 * FZ_H;
     std::vector<double> dzf(nzt), dzc(nzt, 0.0), idzf(nzt), idzc(nzt, 0.0), igz(nzt, 0.0);
@@ -285,12 +279,9 @@ extern "C" fizzy_status fizzy_create(const fizzy_grid *grid, const fizzy_bc *bc,
     k_tri_tables<<<(unsigned)((c->M + 127) / 128), 128, 0, c->stream>>>(P, c->tri);
     FZ_LAUNCHED(FZK_OTHER);
 
-    // dynamic shared memory opt-in for the FFT kernels
+    // dynamic shared memory opt-in (the FFT kernels opt in at launch, per instantiation)
     FZ_CUDA(cudaFuncSetAttribute(k_iface_march<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)IFACE_SMEM));
     FZ_CUDA(cudaFuncSetAttribute(k_iface_march<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)IFACE_SMEM));
-    FZ_CUDA(cudaFuncSetAttribute(k_fftx_fwd<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_x));
-    FZ_CUDA(cudaFuncSetAttribute(k_fftx_fwd<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_x));
-    FZ_CUDA(cudaFuncSetAttribute(k_fftx_inv, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_x));
     return FIZZY_OK;
 }
 
@@ -404,12 +395,9 @@ fizzy_status run_spectral_solve(fizzy_ctx *c, double *dst)
     FZ_CUDA(c->cyclic ? fz_spec_launch<true>(false, c->log2ny, P, c->tri, c->spec, c->twy, c->scal, c->stream)
                       : fz_spec_launch<false>(false, c->log2ny, P, c->tri, c->spec, c->twy, c->scal, c->stream));
     FZ_LAUNCHED(FZK_SPEC_BWD);
-    const long long nlines = (long long)P.ny * P.nz;
-    const unsigned gx = (unsigned)((nlines + 2 * c->Sx - 1) / (2 * c->Sx));
-    const int tx = c->Sx * P.nx / 8;
     FZ_TB(FZK_FFTX_INV);
-    k_fftx_inv<<<gx, tx, c->smem_x, c->stream>>>(P, c->spec, dst, 1.0 / ((double)P.nx * (double)P.ny), c->twx,
-                                                 c->log2nx, c->Sx, c->scal);
+    FZ_CUDA(fz_fftx_launch(2, c->log2nx, P, nullptr, nullptr, nullptr, nullptr, 1.0 / ((double)P.nx * (double)P.ny),
+                           c->spec, dst, c->twx, c->scal, c->stream));
     FZ_LAUNCHED(FZK_FFTX_INV);
     return FIZZY_OK;
 }
@@ -532,12 +520,9 @@ extern "C" fizzy_status fizzy_rk3_substep(fizzy_ctx *c, int stage, double dt)
     else { if (c->varmu) launch_momentum<false, true>(c, grid, block, A); else launch_momentum<false, false>(c, grid, block, A); }
     FZ_LAUNCHED(FZK_MOM);
     // S4: b = rho0/(a dt) D(u**), FFT x (fused), FFT y, tridiagonal z, inverse
-    const long long nlines = (long long)P.ny * P.nz;
-    const unsigned gx = (unsigned)((nlines + 2 * c->Sx - 1) / (2 * c->Sx));
     FZ_TB(FZK_FFTX_FWD);
-    k_fftx_fwd<true><<<gx, c->Sx * P.nx / 8, c->smem_x, c->stream>>>(P, nullptr, c->us, c->vs, c->ws,
-                                                                     P.rho0 / (as * dt), c->spec, c->twx,
-                                                                     c->log2nx, c->Sx);
+    FZ_CUDA(fz_fftx_launch(0, c->log2nx, P, nullptr, c->us, c->vs, c->ws, P.rho0 / (as * dt), c->spec, nullptr,
+                           c->twx, c->scal, c->stream));
     FZ_LAUNCHED(FZK_FFTX_FWD);
     if ((s = run_spectral_solve(c, c->pn)) != FIZZY_OK) return s;
     // S5: correction, pressure rotation
@@ -564,11 +549,9 @@ extern "C" fizzy_status fizzy_poisson_solve(fizzy_ctx *c, const double *rhs, dou
     const FzP &P = c->P;
     const size_t B = (size_t)c->N * sizeof(double);
     FZ_CUDA(cudaMemcpyAsync(c->pn, rhs, B, cudaMemcpyDefault, c->stream));
-    const long long nlines = (long long)P.ny * P.nz;
-    const unsigned gx = (unsigned)((nlines + 2 * c->Sx - 1) / (2 * c->Sx));
     FZ_TB(FZK_FFTX_FWD);
-    k_fftx_fwd<false><<<gx, c->Sx * P.nx / 8, c->smem_x, c->stream>>>(P, c->pn, nullptr, nullptr, nullptr, 1.0,
-                                                                      c->spec, c->twx, c->log2nx, c->Sx);
+    FZ_CUDA(fz_fftx_launch(1, c->log2nx, P, c->pn, nullptr, nullptr, nullptr, 1.0, c->spec, nullptr, c->twx, c->scal,
+                           c->stream));
     FZ_LAUNCHED(FZK_FFTX_FWD);
     fizzy_status s = run_spectral_solve(c, c->pn);
     if (s != FIZZY_OK) return s;

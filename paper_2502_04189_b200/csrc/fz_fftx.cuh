@@ -1,0 +1,157 @@
+// fz_fftx.cuh -- S4a + S4b (x part) and S4d (x part): Poisson right-hand side and the real<->complex
+// FFTs along x (kernel group (c) of BASELINE.json:5; "fast direct FFT solver").
+//
+// Two real lines (j, j+1) are transformed as one complex line z = a + i b by a group of nx/8
+// threads (FzLineFFT: twiddles in registers, padded out-of-place passes); a CTA holds FX_PAIRS
+// groups = 2*FX_PAIRS consecutive j lines of one plane k, so that the half-spectrum goes out in
+// runs of 2*FX_PAIRS consecutive j:  spec[(k*nxh + l)*ny + j]  (y lines contiguous, fz_spectral.cuh).
+//   A_l = (Z_l + conj Z_{n-l})/2,  B_l = (Z_l - conj Z_{n-l})/(2i)          (forward untangling)
+//   Z_l = A_l + i B_l,  Z_{n-l} = conj(A_l) + i conj(B_l)                   (backward tangling)
+// DIV = true: the real input is the Poisson right-hand side assembled on the fly,
+//   b = coef * D(u**)  (BASELINE.json:5(iv) with the p_hat term folded into u**, D2);
+// DIV = false: the real input is read from `src` (fizzy_poisson_solve).
+#pragma once
+#include "fz_common.cuh"
+#include "fz_linefft.cuh"
+
+#define FX_PAIRS 4
+#define FX_LINE(n_) ((n_) + ((n_) >> 3))
+
+__host__ __device__ inline size_t fz_fftx_smem(int n) { return (size_t)2 * FX_PAIRS * FX_LINE(n) * 16; }
+
+template <bool DIV, int LOG2N>
+__global__ void __launch_bounds__(FX_PAIRS * 128)
+k_fftx_fwd(FzP P, const double *__restrict__ src, const double *__restrict__ us,
+           const double *__restrict__ vs, const double *__restrict__ ws, double coef,
+           double2 *__restrict__ spec, const double2 *__restrict__ tw)
+{
+    extern __shared__ __align__(16) double2 smx[];
+    constexpr int n = 1 << LOG2N, T8 = n / 8, LN = FX_LINE(n);
+    const int jt = threadIdx.x, g = threadIdx.y;
+    double2 *A = smx + (2 * g) * LN, *B = A + LN;
+    FzLineFFT<LOG2N, -1> fft;
+    fft.init(tw, jt);
+    const long long L0 = (long long)blockIdx.x * (2 * FX_PAIRS);   // first line of the CTA; 2*FX_PAIRS | ny
+    const int k = (int)(L0 / P.ny), j0 = (int)(L0 - (long long)k * P.ny);
+    const int ja = j0 + 2 * g;                                      // lines ja (real part), ja+1 (imaginary part)
+    const long long ra = ((long long)k * P.ny + ja) * n, rb = ra + n;
+    double2 v[8];
+    if (DIV) {
+        const long long rm = ((long long)k * P.ny + fz_im(ja, P.ny)) * n;   // row ja-1 (periodic)
+        const bool wall_lo = P.z_wall && k == 0;
+        const long long dzl = (k == 0) ? (long long)(P.nz - 1) * P.sxy : -P.sxy;   // plane k-1 (periodic wrap)
+        const double izf = P.idzf[k];
+#pragma unroll
+        for (int q = 0; q < 8; ++q) {
+            const int i = jt + q * T8, im = fz_im(i, n);
+            const double va = vs[ra + i];
+            const double wla = wall_lo ? 0.0 : ws[ra + i + dzl], wlb = wall_lo ? 0.0 : ws[rb + i + dzl];
+            v[q].x = coef * ((us[ra + i] - us[ra + im]) * P.idx + (va - vs[rm + i]) * P.idy + (ws[ra + i] - wla) * izf);
+            v[q].y = coef * ((us[rb + i] - us[rb + im]) * P.idx + (vs[rb + i] - va) * P.idy + (ws[rb + i] - wlb) * izf);
+        }
+    } else {
+#pragma unroll
+        for (int q = 0; q < 8; ++q) { const int i = jt + q * T8; v[q] = make_double2(src[ra + i], src[rb + i]); }
+    }
+    const double2 *res = fft.regs_to_smem(jt, A, B, v);   // same buffer (A or B) in every group
+    const int roff = (int)(res - A);
+    // untangle and store: consecutive threads -> consecutive j (runs of 2*FX_PAIRS*16 bytes)
+    const int nth = T8 * FX_PAIRS, t = g * T8 + jt;
+    const int nxh = P.nxh;
+    double2 *out = spec + (long long)k * nxh * P.ny + j0;
+    for (int e = t; e < 2 * FX_PAIRS * nxh; e += nth) {
+        const int l = e / (2 * FX_PAIRS), ln = e - l * (2 * FX_PAIRS);
+        const double2 *buf = smx + (2 * (ln >> 1)) * LN + roff;
+        const double2 z1 = buf[FZL_PADI(l)];
+        const int l2 = (n - l) & (n - 1);
+        const double2 z2 = buf[FZL_PADI(l2)];
+        double2 o;
+        if (ln & 1) o = make_double2(0.5 * (z1.y + z2.y), -0.5 * (z1.x - z2.x));  // B_l
+        else o = make_double2(0.5 * (z1.x + z2.x), 0.5 * (z1.y - z2.y));          // A_l
+        out[(long long)l * P.ny + ln] = o;
+    }
+}
+
+// ---------------------------------------------------------------- FFT along x, backward (c2r)
+// out = Re / Im of the inverse transform * scale - gauge shift (N17: scal[2] = mean of mode (0,0),
+// written by k_spec_bwd)
+template <int LOG2N>
+__global__ void __launch_bounds__(FX_PAIRS * 128)
+k_fftx_inv(FzP P, const double2 *__restrict__ spec, double *__restrict__ dst, double scale,
+           const double2 *__restrict__ tw, const double *__restrict__ scal)
+{
+    extern __shared__ __align__(16) double2 smx[];
+    constexpr int n = 1 << LOG2N, T8 = n / 8, LN = FX_LINE(n);
+    const int jt = threadIdx.x, g = threadIdx.y;
+    double2 *A = smx + (2 * g) * LN, *B = A + LN;
+    FzLineFFT<LOG2N, +1> fft;
+    fft.init(tw, jt);
+    const long long L0 = (long long)blockIdx.x * (2 * FX_PAIRS);
+    const int k = (int)(L0 / P.ny), j0 = (int)(L0 - (long long)k * P.ny);
+    const double shift = scal[2] * scale;
+    const int nth = T8 * FX_PAIRS, t = g * T8 + jt;
+    const int nxh = P.nxh;
+    const double2 *in = spec + (long long)k * nxh * P.ny + j0;
+    // tangle: consecutive threads -> consecutive pairs (32-byte pieces, runs of 2*FX_PAIRS*16 bytes per l)
+    for (int e = t; e < FX_PAIRS * nxh; e += nth) {
+        const int l = e / FX_PAIRS, pr = e - l * FX_PAIRS;
+        const double2 a = in[(long long)l * P.ny + 2 * pr], b = in[(long long)l * P.ny + 2 * pr + 1];
+        double2 *buf = smx + (2 * pr) * LN;
+        if (l == 0 || l == n / 2) {
+            buf[FZL_PADI(l)] = make_double2(a.x, b.x);
+        } else {
+            buf[FZL_PADI(l)] = make_double2(a.x - b.y, a.y + b.x);
+            buf[FZL_PADI(n - l)] = make_double2(a.x + b.y, b.x - a.y);
+        }
+    }
+    __syncthreads();
+    double2 v[8];
+    fft.smem_to_regs(jt, A, B, v);
+    const int ja = j0 + 2 * g;
+    const long long ra = ((long long)k * P.ny + ja) * n, rb = ra + n;
+#pragma unroll
+    for (int q = 0; q < 8; ++q) {
+        const int i = jt + q * T8;
+        dst[ra + i] = v[q].x * scale - shift;
+        dst[rb + i] = v[q].y * scale - shift;
+    }
+}
+
+// ---------------------------------------------------------------- host-side dispatch over log2(nx)
+template <int LOG2N>
+cudaError_t fz_fftx_launch_one(int which /*0 fwd DIV, 1 fwd plain, 2 inv*/, const FzP &P, const double *src,
+                               const double *us, const double *vs, const double *ws, double coef, double2 *spec,
+                               double *dst, const double2 *tw, const double *scal, cudaStream_t st)
+{
+    const int n = 1 << LOG2N;
+    const size_t smem = fz_fftx_smem(n);
+    const dim3 block(n / 8, FX_PAIRS);
+    const unsigned grid = (unsigned)(((long long)P.ny * P.nz) / (2 * FX_PAIRS));
+    cudaError_t e;
+    if (which == 0) {
+        e = cudaFuncSetAttribute(k_fftx_fwd<true, LOG2N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        k_fftx_fwd<true, LOG2N><<<grid, block, smem, st>>>(P, nullptr, us, vs, ws, coef, spec, tw);
+    } else if (which == 1) {
+        e = cudaFuncSetAttribute(k_fftx_fwd<false, LOG2N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        k_fftx_fwd<false, LOG2N><<<grid, block, smem, st>>>(P, src, nullptr, nullptr, nullptr, 1.0, spec, tw);
+    } else {
+        e = cudaFuncSetAttribute(k_fftx_inv<LOG2N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        k_fftx_inv<LOG2N><<<grid, block, smem, st>>>(P, spec, dst, coef, tw, scal);
+    }
+    return cudaSuccess;
+}
+
+inline cudaError_t fz_fftx_launch(int which, int log2n, const FzP &P, const double *src, const double *us,
+                                  const double *vs, const double *ws, double coef, double2 *spec, double *dst,
+                                  const double2 *tw, const double *scal, cudaStream_t st)
+{
+    switch (log2n) {
+#define FZ_CASE(L_) case L_: return fz_fftx_launch_one<L_>(which, P, src, us, vs, ws, coef, spec, dst, tw, scal, st);
+        FZ_CASE(3) FZ_CASE(4) FZ_CASE(5) FZ_CASE(6) FZ_CASE(7) FZ_CASE(8) FZ_CASE(9) FZ_CASE(10)
+#undef FZ_CASE
+    }
+    return cudaErrorInvalidValue;
+}

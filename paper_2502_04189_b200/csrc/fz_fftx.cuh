@@ -15,12 +15,15 @@
 #include "fz_linefft.cuh"
 
 #define FX_PAIRS 4
+#ifndef FX_MINB
+#define FX_MINB 3
+#endif
 #define FX_LINE(n_) ((n_) + ((n_) >> 3))
 
 __host__ __device__ inline size_t fz_fftx_smem(int n) { return (size_t)2 * FX_PAIRS * FX_LINE(n) * 16; }
 
 template <bool DIV, int LOG2N>
-__global__ void __launch_bounds__(FX_PAIRS * 128)
+__global__ void __launch_bounds__(FX_PAIRS * ((1 << LOG2N) / 8), LOG2N <= 9 ? FX_MINB : 1)
 k_fftx_fwd(FzP P, const double *__restrict__ src, const double *__restrict__ us,
            const double *__restrict__ vs, const double *__restrict__ ws, double coef,
            double2 *__restrict__ spec, const double2 *__restrict__ tw)
@@ -29,7 +32,7 @@ k_fftx_fwd(FzP P, const double *__restrict__ src, const double *__restrict__ us,
     constexpr int n = 1 << LOG2N, T8 = n / 8, LN = FX_LINE(n);
     const int jt = threadIdx.x, g = threadIdx.y;
     double2 *A = smx + (2 * g) * LN, *B = A + LN;
-    FzLineFFT<LOG2N, -1> fft;
+    FzLineFFT<LOG2N, -1, false> fft;
     fft.init(tw, jt);
     const long long L0 = (long long)blockIdx.x * (2 * FX_PAIRS);   // first line of the CTA; 2*FX_PAIRS | ny
     const int k = (int)(L0 / P.ny), j0 = (int)(L0 - (long long)k * P.ny);
@@ -76,7 +79,7 @@ k_fftx_fwd(FzP P, const double *__restrict__ src, const double *__restrict__ us,
 // out = Re / Im of the inverse transform * scale - gauge shift (N17: scal[2] = mean of mode (0,0),
 // written by k_spec_bwd)
 template <int LOG2N>
-__global__ void __launch_bounds__(FX_PAIRS * 128)
+__global__ void __launch_bounds__(FX_PAIRS * ((1 << LOG2N) / 8), LOG2N <= 9 ? FX_MINB : 1)
 k_fftx_inv(FzP P, const double2 *__restrict__ spec, double *__restrict__ dst, double scale,
            const double2 *__restrict__ tw, const double *__restrict__ scal)
 {
@@ -84,7 +87,7 @@ k_fftx_inv(FzP P, const double2 *__restrict__ spec, double *__restrict__ dst, do
     constexpr int n = 1 << LOG2N, T8 = n / 8, LN = FX_LINE(n);
     const int jt = threadIdx.x, g = threadIdx.y;
     double2 *A = smx + (2 * g) * LN, *B = A + LN;
-    FzLineFFT<LOG2N, +1> fft;
+    FzLineFFT<LOG2N, +1, false> fft;
     fft.init(tw, jt);
     const long long L0 = (long long)blockIdx.x * (2 * FX_PAIRS);
     const int k = (int)(L0 / P.ny), j0 = (int)(L0 - (long long)k * P.ny);

@@ -12,17 +12,29 @@
 
 #define FZL_PADI(i_) ((i_) + ((i_) >> 3))
 
-template <int LOG2N, int SGN>
+// TWREG = false: a thread that transforms only one line reads its twiddles from the table when a pass
+// needs them (L1 hits) instead of holding them in registers.
+template <int LOG2N, int SGN, bool TWREG = true>
 struct FzLineFFT {
     static constexpr int N = 1 << LOG2N, NP8 = LOG2N / 3, REM = LOG2N % 3, T8 = N / 8;
     static constexpr int R2 = 1 << REM, NB = 8 / R2;          // remainder pass: radix R2, NB butterflies per thread
     static constexpr bool OUT_IN_REGS = (REM == 0);
-    double2 w8[NP8 > 1 ? NP8 - 1 : 1][7];
-    double2 wr[REM ? NB : 1][REM ? R2 - 1 : 1];
+    double2 w8[(TWREG && NP8 > 1) ? NP8 - 1 : 1][7];
+    double2 wr[(TWREG && REM) ? NB : 1][REM ? R2 - 1 : 1];
+    const double2 *twp;
+
+    __device__ __forceinline__ double2 twv(int q) const
+    {
+        double2 t = twp[q];
+        if (SGN > 0) t.y = -t.y;
+        return t;
+    }
 
     // tw[q] = exp(-2 pi i q / N); jt = thread index within the line
     __device__ __forceinline__ void init(const double2 *__restrict__ tw, int jt)
     {
+        twp = tw;
+        if (!TWREG) return;
         int Ns = 8;
 #pragma unroll
         for (int p = 1; p < NP8; ++p) {
@@ -58,8 +70,9 @@ struct FzLineFFT {
             for (int r = 0; r < 8; ++r) v[r] = src[FZL_PADI(jt + r * T8)];
         }
         if (p > 0) {
+            const int Nsp = 1 << (3 * p), kt = (jt & (Nsp - 1)) * (N / (Nsp * 8));
 #pragma unroll
-            for (int r = 1; r < 8; ++r) v[r] = fz_cmul(v[r], w8[p - 1][r - 1]);
+            for (int r = 1; r < 8; ++r) v[r] = fz_cmul(v[r], TWREG ? w8[p - 1][r - 1] : twv(r * kt));
         }
         fz_dft8<SGN>(v);
         if (!OUT_REG) {
@@ -81,7 +94,7 @@ struct FzLineFFT {
 #pragma unroll
             for (int r = 0; r < R2; ++r) u[r] = src[FZL_PADI(j + r * T)];
 #pragma unroll
-            for (int r = 1; r < R2; ++r) u[r] = fz_cmul(u[r], wr[b][r - 1]);
+            for (int r = 1; r < R2; ++r) u[r] = fz_cmul(u[r], TWREG ? wr[b][r - 1] : twv(r * j));
             if constexpr (R2 == 4) fz_dft4<SGN>(u[0], u[1], u[2], u[3]);
             else fz_dft2<SGN>(u[0], u[1]);
             const int kk = j & (Ns - 1), base = (j - kk) * R2 + kk;

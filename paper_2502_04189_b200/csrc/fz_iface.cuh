@@ -90,7 +90,8 @@ k_iface_march(FzP P, const double *__restrict__ psi, const double *__restrict__ 
         const double gx = (PSI[o0 + q + 1] - PSI[o0 + q - 1]) * hx;
         const double gy = (PSI[o0 + q + IPW] - PSI[o0 + q - IPW]) * hy;
         const double gz = (PSI[op + q] - PSI[om + q]) * igz;
-        const double inv = fz_rsqrt(fmax(gx * gx + gy * gy + gz * gz, 1e-60));  // 1/max(|G|, 1e-30) (N4)
+        // HALF the normal: 0.5 G / max(|G|, 1e-30) (N4), so that a face normal is a plain sum
+        const double inv = 0.5 * fz_rsqrt(fmax(gx * gx + gy * gy + gz * gz, 1e-60));
         nx_ = gx * inv; ny_ = gy * inv; nz_ = gz * inv;
     };
 
@@ -98,7 +99,7 @@ k_iface_march(FzP P, const double *__restrict__ psi, const double *__restrict__ 
     issue_psi(k0 - 2); issue_psi(k0 - 1); issue_rf(k0 - 2); fz_cp_async_commit();
     issue_psi(k0); issue_rf(k0 - 1); fz_cp_async_commit();
     issue_psi(k0 + 1); issue_rf(k0); fz_cp_async_commit();
-    double nzm = 0.0, nz0 = 0.0, nzp = 0.0, fm = 0.0, rm = 0.0;
+    double nz0 = 0.0, nzp = 0.0, nfz_prev = 0.0, Rz_prev = 0.0;
     const long long gc = (i0 + tx) + (long long)P.nx * (j0 + ty);
     // ring offsets of psi planes kk-1, kk, kk+1 and of the nhat planes kk-1, kk, advanced incrementally
     int sp = (k0 - 3 + 2 * IRING_PSI) % IRING_PSI;   // slot of psi plane kk-2 before the first step
@@ -120,43 +121,38 @@ k_iface_march(FzP P, const double *__restrict__ psi, const double *__restrict__ 
             double ax, ay, az;
             normal(pc, pm, p0, pp, igz, ax, ay, az);
             NHX[n0 + nc] = ax; NHY[n0 + nc] = ay;
-            nzm = nz0; nz0 = nzp; nzp = az;
+            nz0 = nzp; nzp = az;
             if (has_h) {
                 normal(ph, pm, p0, pp, igz, ax, ay, az);
                 NHX[n0 + nh] = ax; NHY[n0 + nh] = ay;
             }
         }
         const int k = kk - 1;
+        if (k < k0 - 1) continue;
         const int rk = ((k + 2 * IRING_RF) & (IRING_RF - 1)) * IPS + pc;    // r, phi plane k, own cell
         const int rp = ((kk + 2 * IRING_RF) & (IRING_RF - 1)) * IPS + pc;   // plane k+1
-        // phi, r of plane k-1 travel in registers (fm, rm)
         const double f0 = PHI[rk], r0 = RR[rk];
-        if (k < k0) { fm = f0; rm = r0; continue; }
-        // nhat_x, nhat_y of plane k were written one step ago: visible after this step's barrier
-        const bool gm = P.z_wall && k == 0, gp = P.z_wall && k == P.nz - 1;
+        // z face k+1/2 (between planes k and k+1): zero on a wall face; the face k-1/2 is carried in
+        // registers from the previous step (hz = half the face normal = nf_z)
+        const double zf = (P.z_wall && (k == -1 || k == P.nz - 1)) ? 0.0 : 1.0;
+        const double nfzp = zf * (nz0 + nzp);
+        const double Rzp = zf * (P.eps * (PHI[rp] - f0) * P.idzc[k] - fz_sharp2(r0, RR[rp]) * nfzp);
+        if (k < k0) { nfz_prev = nfzp; Rz_prev = Rzp; continue; }
+        // half normals of plane k were written one step ago: visible after this step's barrier
         const double ax = NHX[nm + nc], ay = NHY[nm + nc];
-        const double nfxp = 0.5 * (ax + NHX[nm + nc + 1]), nfxm = 0.5 * (NHX[nm + nc - 1] + ax);
-        const double nfyp = 0.5 * (ay + NHY[nm + nc + INW]), nfym = 0.5 * (NHY[nm + nc - INW] + ay);
+        const double nfxp = ax + NHX[nm + nc + 1], nfxm = NHX[nm + nc - 1] + ax;
+        const double nfyp = ay + NHY[nm + nc + INW], nfym = NHY[nm + nc - INW] + ay;
         const double ex = P.eps * P.idx, ey = P.eps * P.idy;
         const double Rxp = ex * (PHI[rk + 1] - f0) - fz_sharp2(r0, RR[rk + 1]) * nfxp;
         const double Rxm = ex * (f0 - PHI[rk - 1]) - fz_sharp2(RR[rk - 1], r0) * nfxm;
         const double Ryp = ey * (PHI[rk + IPW] - f0) - fz_sharp2(r0, RR[rk + IPW]) * nfyp;
         const double Rym = ey * (f0 - PHI[rk - IPW]) - fz_sharp2(RR[rk - IPW], r0) * nfym;
-        double nfzp = 0.0, nfzm = 0.0, Rzp = 0.0, Rzm = 0.0;
-        if (!gp) {
-            nfzp = 0.5 * (nz0 + nzp);
-            Rzp = P.eps * (PHI[rp] - f0) * P.idzc[k] - fz_sharp2(r0, RR[rp]) * nfzp;
-        }
-        if (!gm) {
-            nfzm = 0.5 * (nzm + nz0);
-            Rzm = P.eps * (f0 - fm) * P.idzc[k - 1] - fz_sharp2(rm, r0) * nfzm;
-        }
         const double izf = P.idzf[k];
         const long long c = (long long)k * P.sxy + gc;
-        kappa[c] = -((nfxp - nfxm) * P.idx + (nfyp - nfym) * P.idy + (nfzp - nfzm) * izf);
-        divrn[c] = (Rxp - Rxm) * P.idx + (Ryp - Rym) * P.idy + (Rzp - Rzm) * izf;
+        kappa[c] = -((nfxp - nfxm) * P.idx + (nfyp - nfym) * P.idy + (nfzp - nfz_prev) * izf);
+        divrn[c] = (Rxp - Rxm) * P.idx + (Ryp - Rym) * P.idy + (Rzp - Rz_prev) * izf;
         if (STORE_R) { rnx[c] = Rxp; rny[c] = Ryp; rnz[c] = Rzp; }
-        fm = f0; rm = r0;
+        nfz_prev = nfzp; Rz_prev = Rzp;
     }
     fz_cp_async_wait<0>();
 }

@@ -219,7 +219,7 @@ k_momentum_march(FzP P, FzMomArgs A, int KC)
 {
     using F = FzMomFields<VARRHO, HEAT>;
     constexpr int NF = F::NF;
-    extern __shared__ __align__(16) double smm[];  // [NF][MRING][MPS]
+    extern __shared__ __align__(16) double smm[];  // [NF][MRING][MPS] fields | [3][MRING][MTX*MTY] histories
     const int tx = threadIdx.x, ty = threadIdx.y, t = ty * MTX + tx;
     const int i0 = blockIdx.x * MTX, j0 = blockIdx.y * MTY;
     const int i = i0 + tx, j = j0 + ty;
@@ -233,6 +233,7 @@ k_momentum_march(FzP P, FzMomArgs A, int KC)
                              (long long)P.nx * ((j0 - 1 + lrow + P.ny) & (P.ny - 1));
     const int soff = lrow * MPW + 2 * lcp;
 
+    double *hst = smm + NF * (MRING * MPS);   // [3][MRING][MTX*MTY] staged RK histories
     const double *src[NF];
     src[F::U] = A.u; src[F::V] = A.v; src[F::W] = A.w; src[F::PHI] = A.phi; src[F::KAP] = A.kappa;
     if (HEAT) src[F::T] = A.T;
@@ -248,6 +249,14 @@ k_momentum_march(FzP P, FzMomArgs A, int KC)
             const int o = ((kk + MRING) % MRING) * MPS + soff;
 #pragma unroll
             for (int f = 0; f < NF; ++f) fz_cp_async16(smm + f * (MRING * MPS) + o, src[f] + g);
+        }
+        // RK history of the thread's own cell (read back by the same thread only)
+        if (kk >= k0 && kk < k1) {
+            const long long g = (long long)kk * P.sxy + goff_c;
+            double *h = hst + ((kk + MRING) % MRING) * (MTX * MTY) + t;
+            fz_cp_async8(h, A.hu + g);
+            fz_cp_async8(h + MRING * MTX * MTY, A.hv + g);
+            fz_cp_async8(h + 2 * MRING * MTX * MTY, A.hw + g);
         }
     };
     issue(k0 - 1); issue(k0); fz_cp_async_commit();
@@ -270,7 +279,9 @@ k_momentum_march(FzP P, FzMomArgs A, int KC)
         sl = (sl + 1 == MRING) ? 0 : sl + 1;
         om = o0; o0 = op; op = sl * MPS + cidx;   // planes k-1, k, k+1
         const long long c = (long long)k * P.sxy + goff_c;
-        const double hu_old = A.hu[c], hv_old = A.hv[c], hw_old = A.hw[c];
+        const int s0 = (sl == 0) ? MRING - 1 : sl - 1;   // ring slot of plane k
+        const double hu_old = hst[s0 * (MTX * MTY) + t], hv_old = hst[(MRING + s0) * (MTX * MTY) + t],
+                     hw_old = hst[(2 * MRING + s0) * (MTX * MTY) + t];
         // ghost rules at the walls: planes k-1 / k+1 hold the mirrored interior plane
         const bool gm = P.z_wall && k == 0, gp = P.z_wall && k == P.nz - 1;
         const double sgm = gm ? -1.0 : 1.0, sgp = gp ? -1.0 : 1.0, wm = gm ? 0.0 : 1.0;
@@ -317,19 +328,25 @@ k_momentum_march(FzP P, FzMomArgs A, int KC)
         }
         double T000 = 0;
         if (HEAT) T000 = S_(F::T, 0, 0, o0);
+        // edge viscosity (N11): mean of the four cells around the edge; a constant if mu1 == mu2
+#define MUE_(a_, b_, c_, d_) (VARMU ? 0.25 * ((a_) + (b_) + (c_) + (d_)) : P.mu2)
+        // advective edge products and edge stresses on the three "+" edges of the cell, shared by
+        // the two components that meet there
+        const double Exy_p = 0.5 * (v000 + vp00) * 0.5 * (u000 + u0p0);
+        const double Exz_p = 0.5 * (w000 + wp00) * 0.5 * (u000 + u00p);
+        const double Eyz_p = 0.5 * (w000 + w0p0) * 0.5 * (v000 + v00p);
+        const double txy_p = MUE_(m000, mp00, m0p0, mpp0) * ((u0p0 - u000) * dy + (vp00 - v000) * dx);
+        const double txz_p = MUE_(m000, mp00, m00p, mp0p) * ((u00p - u000) * izc + (wp00 - w000) * dx);
+        const double tyz_p = MUE_(m000, m0p0, m00p, m0pp) * ((v00p - v000) * izc + (w0p0 - w000) * dy);
         // ================= x component =================
         {
             const double uc_p = 0.5 * (up00 + u000), uc_m = 0.5 * (u000 + um00);
-            const double Exy_p = 0.5 * (v000 + vp00) * 0.5 * (u000 + u0p0);
             const double Exy_m = 0.5 * (v0m0 + vpm0) * 0.5 * (u0m0 + u000);
-            const double Exz_p = 0.5 * (w000 + wp00) * 0.5 * (u000 + u00p);
             const double Exz_m = 0.5 * (w00m + wp0m) * 0.5 * (u00m + u000);
             const double Aa = -(uc_p * uc_p - uc_m * uc_m) * dx - (Exy_p - Exy_m) * dy - (Exz_p - Exz_m) * izf;
             const double nrm_p = 2.0 * mp00 * (up00 - u000) * dx, nrm_m = 2.0 * m000 * (u000 - um00) * dx;
-            const double txy_p = 0.25 * (m000 + mp00 + m0p0 + mpp0) * ((u0p0 - u000) * dy + (vp00 - v000) * dx);
-            const double txy_m = 0.25 * (m0m0 + mpm0 + m000 + mp00) * ((u000 - u0m0) * dy + (vpm0 - v0m0) * dx);
-            const double txz_p = 0.25 * (m000 + mp00 + m00p + mp0p) * ((u00p - u000) * izc + (wp00 - w000) * dx);
-            const double txz_m = 0.25 * (m00m + mp0m + m000 + mp00) * ((u000 - u00m) * izcm + (wp0m - w00m) * dx);
+            const double txy_m = MUE_(m0m0, mpm0, m000, mp00) * ((u000 - u0m0) * dy + (vpm0 - v0m0) * dx);
+            const double txz_m = MUE_(m00m, mp0m, m000, mp00) * ((u000 - u00m) * izcm + (wp0m - w00m) * dx);
             const double V = (nrm_p - nrm_m) * dx + (txy_p - txy_m) * dy + (txz_p - txz_m) * izf;
             const double Sf = P.sigma * 0.5 * (kap0 + S_(F::KAP, 1, 0, o0)) * (fp00 - f000) * dx;
             double M = 0.0;
@@ -350,16 +367,14 @@ k_momentum_march(FzP P, FzMomArgs A, int KC)
         // ================= y component =================
         {
             const double vc_p = 0.5 * (v0p0 + v000), vc_m = 0.5 * (v000 + v0m0);
-            const double Eyx_p = 0.5 * (u000 + u0p0) * 0.5 * (v000 + vp00);
+            const double Eyx_p = Exy_p;
             const double Eyx_m = 0.5 * (um00 + ump0) * 0.5 * (vm00 + v000);
-            const double Eyz_p = 0.5 * (w000 + w0p0) * 0.5 * (v000 + v00p);
             const double Eyz_m = 0.5 * (w00m + w0pm) * 0.5 * (v00m + v000);
             const double Aa = -(vc_p * vc_p - vc_m * vc_m) * dy - (Eyx_p - Eyx_m) * dx - (Eyz_p - Eyz_m) * izf;
             const double nrm_p = 2.0 * m0p0 * (v0p0 - v000) * dy, nrm_m = 2.0 * m000 * (v000 - v0m0) * dy;
-            const double tyx_p = 0.25 * (m000 + m0p0 + mp00 + mpp0) * ((vp00 - v000) * dx + (u0p0 - u000) * dy);
-            const double tyx_m = 0.25 * (mm00 + mmp0 + m000 + m0p0) * ((v000 - vm00) * dx + (ump0 - um00) * dy);
-            const double tyz_p = 0.25 * (m000 + m0p0 + m00p + m0pp) * ((v00p - v000) * izc + (w0p0 - w000) * dy);
-            const double tyz_m = 0.25 * (m00m + m0pm + m000 + m0p0) * ((v000 - v00m) * izcm + (w0pm - w00m) * dy);
+            const double tyx_p = txy_p;
+            const double tyx_m = MUE_(mm00, mmp0, m000, m0p0) * ((v000 - vm00) * dx + (ump0 - um00) * dy);
+            const double tyz_m = MUE_(m00m, m0pm, m000, m0p0) * ((v000 - v00m) * izcm + (w0pm - w00m) * dy);
             const double V = (nrm_p - nrm_m) * dy + (tyx_p - tyx_m) * dx + (tyz_p - tyz_m) * izf;
             const double Sf = P.sigma * 0.5 * (kap0 + S_(F::KAP, 0, 1, o0)) * (f0p0 - f000) * dy;
             double M = 0.0;
@@ -382,16 +397,16 @@ k_momentum_march(FzP P, FzMomArgs A, int KC)
             const double w00p = S_(F::W, 0, 0, op);
             const double izfp = P.idzf[k + 1];
             const double wc_p = 0.5 * (w00p + w000), wc_m = 0.5 * (w000 + w00m);
-            const double Ezx_p = 0.5 * (u000 + u00p) * 0.5 * (w000 + wp00);
+            const double Ezx_p = Exz_p;
             const double Ezx_m = 0.5 * (um00 + um0p) * 0.5 * (wm00 + w000);
-            const double Ezy_p = 0.5 * (v000 + v00p) * 0.5 * (w000 + w0p0);
+            const double Ezy_p = Eyz_p;
             const double Ezy_m = 0.5 * (v0m0 + v0mp) * 0.5 * (w0m0 + w000);
             const double Aa = -(wc_p * wc_p - wc_m * wc_m) * izc - (Ezx_p - Ezx_m) * dx - (Ezy_p - Ezy_m) * dy;
             const double nrm_p = 2.0 * m00p * (w00p - w000) * izfp, nrm_m = 2.0 * m000 * (w000 - w00m) * izf;
-            const double tzx_p = 0.25 * (m000 + m00p + mp00 + mp0p) * ((wp00 - w000) * dx + (u00p - u000) * izc);
-            const double tzx_m = 0.25 * (mm00 + mm0p + m000 + m00p) * ((w000 - wm00) * dx + (um0p - um00) * izc);
-            const double tzy_p = 0.25 * (m000 + m00p + m0p0 + m0pp) * ((w0p0 - w000) * dy + (v00p - v000) * izc);
-            const double tzy_m = 0.25 * (m0m0 + m0mp + m000 + m00p) * ((w000 - w0m0) * dy + (v0mp - v0m0) * izc);
+            const double tzx_p = txz_p;
+            const double tzx_m = MUE_(mm00, mm0p, m000, m00p) * ((w000 - wm00) * dx + (um0p - um00) * izc);
+            const double tzy_p = tyz_p;
+            const double tzy_m = MUE_(m0m0, m0mp, m000, m00p) * ((w000 - w0m0) * dy + (v0mp - v0m0) * izc);
             const double V = (nrm_p - nrm_m) * izc + (tzx_p - tzx_m) * dx + (tzy_p - tzy_m) * dy;
             const double Sf = P.sigma * 0.5 * (kap0 + S_(F::KAP, 0, 0, op)) * (f00p - f000) * izc;
             double M = 0.0;
@@ -413,5 +428,6 @@ k_momentum_march(FzP P, FzMomArgs A, int KC)
             A.hw[c] = 0.0;
         }
 #undef S_
+#undef MUE_
     }
 }

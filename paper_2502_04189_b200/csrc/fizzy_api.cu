@@ -407,7 +407,7 @@ cudaError_t launch_momentum3(fizzy_ctx *c, dim3 grid, dim3 block, const FzMomArg
 {
     const FzP &P = c->P;
     if (P.nx >= MTX && P.ny >= MTY) {   // 2.5-D marching kernel
-        const size_t smem = ((size_t)FzMomFields<VR, HT>::NF * MRING * MPS + 3 * MRING * MTX * MTY) * sizeof(double);
+        const size_t smem = (size_t)FzMomFields<VR, HT>::NF * MRING * MPS * sizeof(double);
         cudaError_t e = cudaFuncSetAttribute(k_momentum_march<VR, VM, HT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
         const int tiles = (P.nx / MTX) * (P.ny / MTY);

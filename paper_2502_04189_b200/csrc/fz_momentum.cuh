@@ -196,6 +196,9 @@ k_momentum(FzP P, FzMomArgs A)
 // flight -- DRAM latency is hidden by the pipeline rather than by occupancy.  One barrier per
 // plane.  Wall ghosts (no-slip: -u, -v; impermeable: w = 0, R_z = 0; mirror: phi, kappa, p_hat)
 // are applied when a ghost plane is READ: the ring holds the mirrored source plane unchanged.
+#ifndef MOM_MINB
+#define MOM_MINB 3
+#endif
 #define MTX 32
 #define MTY 8
 #define MPW (MTX + 4)
@@ -214,12 +217,12 @@ struct FzMomFields {
 };
 
 template <bool VARRHO, bool VARMU, bool HEAT>
-__global__ void __launch_bounds__(MTX * MTY)
+__global__ void __launch_bounds__(MTX * MTY, (VARRHO || HEAT) ? 1 : MOM_MINB)
 k_momentum_march(FzP P, FzMomArgs A, int KC)
 {
     using F = FzMomFields<VARRHO, HEAT>;
     constexpr int NF = F::NF;
-    extern __shared__ __align__(16) double smm[];  // [NF][MRING][MPS] fields | [3][MRING][MTX*MTY] histories
+    extern __shared__ __align__(16) double smm[];  // [NF][MRING][MPS]
     const int tx = threadIdx.x, ty = threadIdx.y, t = ty * MTX + tx;
     const int i0 = blockIdx.x * MTX, j0 = blockIdx.y * MTY;
     const int i = i0 + tx, j = j0 + ty;
@@ -233,7 +236,6 @@ k_momentum_march(FzP P, FzMomArgs A, int KC)
                              (long long)P.nx * ((j0 - 1 + lrow + P.ny) & (P.ny - 1));
     const int soff = lrow * MPW + 2 * lcp;
 
-    double *hst = smm + NF * (MRING * MPS);   // [3][MRING][MTX*MTY] staged RK histories
     const double *src[NF];
     src[F::U] = A.u; src[F::V] = A.v; src[F::W] = A.w; src[F::PHI] = A.phi; src[F::KAP] = A.kappa;
     if (HEAT) src[F::T] = A.T;
@@ -250,14 +252,6 @@ k_momentum_march(FzP P, FzMomArgs A, int KC)
 #pragma unroll
             for (int f = 0; f < NF; ++f) fz_cp_async16(smm + f * (MRING * MPS) + o, src[f] + g);
         }
-        // RK history of the thread's own cell (read back by the same thread only)
-        if (kk >= k0 && kk < k1) {
-            const long long g = (long long)kk * P.sxy + goff_c;
-            double *h = hst + ((kk + MRING) % MRING) * (MTX * MTY) + t;
-            fz_cp_async8(h, A.hu + g);
-            fz_cp_async8(h + MRING * MTX * MTY, A.hv + g);
-            fz_cp_async8(h + 2 * MRING * MTX * MTY, A.hw + g);
-        }
     };
     issue(k0 - 1); issue(k0); fz_cp_async_commit();
     issue(k0 + 1); fz_cp_async_commit();
@@ -271,6 +265,8 @@ k_momentum_march(FzP P, FzMomArgs A, int KC)
     int sl = (k0 - 1 + MRING) % MRING;   // ring slot of plane k-1, advanced incrementally
     int om, o0 = sl * MPS + cidx, op = ((sl + 1) % MRING) * MPS + cidx;
     sl = (sl + 1) % MRING;
+    double hu_nx = A.hu[(long long)k0 * P.sxy + goff_c], hv_nx = A.hv[(long long)k0 * P.sxy + goff_c],
+           hw_nx = A.hw[(long long)k0 * P.sxy + goff_c];
     for (int k = k0; k < k1; ++k) {
         fz_cp_async_wait<1>();
         __syncthreads();
@@ -279,9 +275,9 @@ k_momentum_march(FzP P, FzMomArgs A, int KC)
         sl = (sl + 1 == MRING) ? 0 : sl + 1;
         om = o0; o0 = op; op = sl * MPS + cidx;   // planes k-1, k, k+1
         const long long c = (long long)k * P.sxy + goff_c;
-        const int s0 = (sl == 0) ? MRING - 1 : sl - 1;   // ring slot of plane k
-        const double hu_old = hst[s0 * (MTX * MTY) + t], hv_old = hst[(MRING + s0) * (MTX * MTY) + t],
-                     hw_old = hst[(2 * MRING + s0) * (MTX * MTY) + t];
+        // RK histories: loaded one plane ahead (registers), so their latency hides behind a whole plane
+        const double hu_old = hu_nx, hv_old = hv_nx, hw_old = hw_nx;
+        if (k + 1 < k1) { hu_nx = A.hu[c + P.sxy]; hv_nx = A.hv[c + P.sxy]; hw_nx = A.hw[c + P.sxy]; }
         // ghost rules at the walls: planes k-1 / k+1 hold the mirrored interior plane
         const bool gm = P.z_wall && k == 0, gp = P.z_wall && k == P.nz - 1;
         const double sgm = gm ? -1.0 : 1.0, sgp = gp ? -1.0 : 1.0, wm = gm ? 0.0 : 1.0;

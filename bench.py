@@ -58,6 +58,21 @@ def substep_model_bytes(cfg):
     return 400.0 if cfg["heat"] else 328.0
 
 
+def max_over_ranks(ms, dist, device):
+    """Replicas only: the one collective of the bench is the MAX of the elapsed time."""
+    if dist is None:
+        return float(ms)
+    import torch
+    t = torch.tensor([ms], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_value(world, cells, substeps, ms):
+    """Mcell-substeps/s of all ranks together: every rank advances its own replica of `cells` cells."""
+    return world * cells * substeps / (ms * 1e-3) / 1e6
+
+
 def measured_peak_gbs():
     try:
         with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
@@ -219,11 +234,8 @@ def main():
     fz.fizzy_get_fields(phi=chk)
     torch.cuda.synchronize()
     finite = bool(torch.isfinite(chk).all().item())
-    if dist is not None:
-        t = torch.tensor([ms], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
-    value = world * cells * 3 * args.steps / (ms * 1e-3) / 1e6
+    ms = max_over_ranks(ms, dist, "cuda")
+    value = whole_job_value(world, cells, 3 * args.steps, ms)
 
     # ---------------- roofline of the dominant kernel + per-kernel table ----------------
     peak, peak_src = measured_peak_gbs()
@@ -275,11 +287,8 @@ def main():
         e1.record(fz.stream)
         barrier()
         ems = e0.elapsed_time(e1)
-        if dist is not None:
-            t = torch.tensor([ems], device="cuda", dtype=torch.float64)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            ems = float(t.item())
-        e2e = {"value": world * cells * 3 * ke / (ems * 1e-3) / 1e6, "unit": UNIT,
+        ems = max_over_ranks(ems, dist, "cuda")
+        e2e = {"value": whole_job_value(world, cells, 3 * ke, ems), "unit": UNIT,
                "h2d_bytes_per_step": nb * len(names), "d2h_bytes_per_step": nb * len(names), "steps": ke,
                "note": "fizzy_set_fields(host) + 3 x fizzy_rk3_substep + fizzy_get_fields(host) per step"}
 

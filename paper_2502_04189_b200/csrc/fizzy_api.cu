@@ -81,6 +81,7 @@ bool valid_inputs(const fizzy_grid *g, const fizzy_bc *bc, const fizzy_props *pr
     if (!g || !bc || !pr) return false;
     if (!is_pow2(g->nx) || !is_pow2(g->ny) || g->nx < 8 || g->ny < 8 || g->nx > 1024 || g->ny > 1024) return false;
     if (g->nz < 4) return false;
+    if ((long long)g->nx * g->ny * g->nz >= (1LL << 31)) return false;   // kernels use 32-bit cell offsets
     if (!(g->lx > 0) || !(g->ly > 0) || !(g->lz > 0)) return false;
     if (bc->z_wall != 0 && bc->z_wall != 1) return false;
     if (g->zf) {

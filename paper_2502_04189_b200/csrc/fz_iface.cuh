@@ -63,16 +63,24 @@ k_iface_march(FzP P, const double *__restrict__ psi, const double *__restrict__ 
     const long long goff = ((i0 - 2 + 2 * lcp + P.nx) & (P.nx - 1)) +
                            (long long)P.nx * ((j0 - 2 + lrow + P.ny) & (P.ny - 1));
     const int soff = lrow * IPW + 2 * lcp;
+    // planes are issued in increasing order, so the ring slots advance incrementally; offsets are
+    // 32-bit (fizzy_create guarantees N < 2^31) and the ghost-plane map is branch-free
+    const int zlo = P.z_wall ? -1 : P.nz, zhi = P.z_wall ? 2 * P.nz - 1 : -P.nz, zsg = P.z_wall ? -1 : 1;
+    auto zsrc = [&](int kk) { return kk < 0 ? zlo + zsg * kk : (kk >= P.nz ? zhi + zsg * kk : kk); };
+    const unsigned sxy = (unsigned)P.sxy, ugoff = (unsigned)goff;
+    int sl_psi = (k0 - 2 + 2 * IRING_PSI) % IRING_PSI, sl_rf = (k0 - 2 + 2 * IRING_RF) & (IRING_RF - 1);
     auto issue_psi = [&](int kk) {   // plane kk of psi -> ring slot kk mod 5
-        if (loader) fz_cp_async16(PSI + ((kk + 2 * IRING_PSI) % IRING_PSI) * IPS + soff, psi + (long long)fz_zsrc(P, kk) * P.sxy + goff);
+        if (loader) fz_cp_async16(PSI + sl_psi * IPS + soff, psi + ((unsigned)zsrc(kk) * sxy + ugoff));
+        sl_psi = (sl_psi + 1 == IRING_PSI) ? 0 : sl_psi + 1;
     };
     auto issue_rf = [&](int kk) {    // plane kk of r, phi -> ring slot kk mod 4
         if (loader) {
-            const long long g = (long long)fz_zsrc(P, kk) * P.sxy + goff;
-            const int o = ((kk + 2 * IRING_RF) & (IRING_RF - 1)) * IPS + soff;
+            const unsigned g = (unsigned)zsrc(kk) * sxy + ugoff;
+            const int o = sl_rf * IPS + soff;
             fz_cp_async16(RR + o, rr + g);
             fz_cp_async16(PHI + o, phi + g);
         }
+        sl_rf = (sl_rf + 1) & (IRING_RF - 1);
     };
     // halo-1 cross cell of the nhat plane handled by this thread (threads 0 .. 2(ITX+ITY)-1)
     int hr = 1, hc = 2;

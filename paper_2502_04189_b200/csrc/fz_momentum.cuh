@@ -241,17 +241,21 @@ k_momentum_march(FzP P, FzMomArgs A, int KC)
     if (HEAT) src[F::T] = A.T;
     if (VARRHO) { src[F::RX] = A.rnx; src[F::RY] = A.rny; src[F::RZ] = A.rnz; src[F::PN] = A.p; src[F::PO] = A.pp; }
 
-    // copy plane kk (k0-1 .. k1; ghosts: periodic wrap or wall mirror) of every field into ring slot kk mod 5
+    // copy plane kk (k0-1 .. k1; ghosts: periodic wrap or wall mirror) of every field into ring slot
+    // kk mod 5.  Planes are issued in increasing order: the slot advances incrementally; offsets are
+    // 32-bit (fizzy_create guarantees N < 2^31).
+    const unsigned sxy = (unsigned)P.sxy, ugoff = (unsigned)goff_l;
+    const int zlo = P.z_wall ? 0 : P.nz - 1, zhi = P.z_wall ? P.nz - 1 : 0;   // source of plane -1 / nz
+    int sl_is = (k0 - 1 + MRING) % MRING;
     auto issue = [&](int kk) {
         if (loader && kk <= k1) {
-            int sp = kk;
-            if (P.z_wall) sp = kk < 0 ? 0 : (kk >= P.nz ? P.nz - 1 : kk);
-            else sp = kk < 0 ? kk + P.nz : (kk >= P.nz ? kk - P.nz : kk);
-            const long long g = (long long)sp * P.sxy + goff_l;
-            const int o = ((kk + MRING) % MRING) * MPS + soff;
+            const int sp = kk < 0 ? zlo : (kk >= P.nz ? zhi : kk);
+            const unsigned g = (unsigned)sp * sxy + ugoff;
+            const int o = sl_is * MPS + soff;
 #pragma unroll
             for (int f = 0; f < NF; ++f) fz_cp_async16(smm + f * (MRING * MPS) + o, src[f] + g);
         }
+        sl_is = (sl_is + 1 == MRING) ? 0 : sl_is + 1;
     };
     issue(k0 - 1); issue(k0); fz_cp_async_commit();
     issue(k0 + 1); fz_cp_async_commit();

@@ -114,6 +114,7 @@ k_iface_march(FzP P, const double *__restrict__ psi, const double *__restrict__ 
     int pm, p0 = ((sp + 1) % IRING_PSI) * IPS, pp = ((sp + 2) % IRING_PSI) * IPS;
     sp = (sp + 2) % IRING_PSI;                       // slot of plane kk (kk = k0-2 "before" the loop)
     int sn = (k0 - 2 + INRING) % INRING, n0 = sn * INS, nm;
+    double igz_n = P.igz[k0 - 1], idzc_n = P.idzc[k0 - 2], idzf_n = P.idzf[k0 - 2];   // z metrics: one step ahead
     for (int kk = k0 - 1; kk <= k1; ++kk) {
         fz_cp_async_wait<1>();
         __syncthreads();
@@ -125,7 +126,8 @@ k_iface_march(FzP P, const double *__restrict__ psi, const double *__restrict__ 
         sn = (sn + 1 == INRING) ? 0 : sn + 1;
         nm = n0; n0 = sn * INS;                      // nhat planes kk-1, kk
         {   // nhat(kk): own cell, then the halo cross
-            const double igz = P.igz[kk];
+            const double igz = igz_n;
+            igz_n = P.igz[kk + 1];
             double ax, ay, az;
             normal(pc, pm, p0, pp, igz, ax, ay, az);
             NHX[n0 + nc] = ax; NHY[n0 + nc] = ay;
@@ -136,6 +138,8 @@ k_iface_march(FzP P, const double *__restrict__ psi, const double *__restrict__ 
             }
         }
         const int k = kk - 1;
+        const double idzc_k = idzc_n, idzf_k = idzf_n;   // metrics of plane k, loaded one step ago
+        idzc_n = P.idzc[kk]; idzf_n = P.idzf[kk];
         if (k < k0 - 1) continue;
         const int rk = ((k + 2 * IRING_RF) & (IRING_RF - 1)) * IPS + pc;    // r, phi plane k, own cell
         const int rp = ((kk + 2 * IRING_RF) & (IRING_RF - 1)) * IPS + pc;   // plane k+1
@@ -144,7 +148,7 @@ k_iface_march(FzP P, const double *__restrict__ psi, const double *__restrict__ 
         // registers from the previous step (hz = half the face normal = nf_z)
         const double zf = (P.z_wall && (k == -1 || k == P.nz - 1)) ? 0.0 : 1.0;
         const double nfzp = zf * (nz0 + nzp);
-        const double Rzp = zf * (P.eps * (PHI[rp] - f0) * P.idzc[k] - fz_sharp2(r0, RR[rp]) * nfzp);
+        const double Rzp = zf * (P.eps * (PHI[rp] - f0) * idzc_k - fz_sharp2(r0, RR[rp]) * nfzp);
         if (k < k0) { nfz_prev = nfzp; Rz_prev = Rzp; continue; }
         // half normals of plane k were written one step ago: visible after this step's barrier
         const double ax = NHX[nm + nc], ay = NHY[nm + nc];
@@ -155,7 +159,7 @@ k_iface_march(FzP P, const double *__restrict__ psi, const double *__restrict__ 
         const double Rxm = ex * (f0 - PHI[rk - 1]) - fz_sharp2(RR[rk - 1], r0) * nfxm;
         const double Ryp = ey * (PHI[rk + IPW] - f0) - fz_sharp2(r0, RR[rk + IPW]) * nfyp;
         const double Rym = ey * (f0 - PHI[rk - IPW]) - fz_sharp2(RR[rk - IPW], r0) * nfym;
-        const double izf = P.idzf[k];
+        const double izf = idzf_k;
         const long long c = (long long)k * P.sxy + gc;
         kappa[c] = -((nfxp - nfxm) * P.idx + (nfyp - nfym) * P.idy + (nfzp - nfz_prev) * izf);
         divrn[c] = (Rxp - Rxm) * P.idx + (Ryp - Rym) * P.idy + (Rzp - Rz_prev) * izf;

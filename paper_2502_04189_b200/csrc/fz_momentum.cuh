@@ -271,6 +271,7 @@ k_momentum_march(FzP P, FzMomArgs A, int KC)
     sl = (sl + 1) % MRING;
     double hu_nx = A.hu[(long long)k0 * P.sxy + goff_c], hv_nx = A.hv[(long long)k0 * P.sxy + goff_c],
            hw_nx = A.hw[(long long)k0 * P.sxy + goff_c];
+    double izc_0 = P.idzc[k0 - 1], izc_n = P.idzc[k0], izf_p = P.idzf[k0], izf_n = P.idzf[k0 + 1];
     for (int k = k0; k < k1; ++k) {
         fz_cp_async_wait<1>();
         __syncthreads();
@@ -287,7 +288,11 @@ k_momentum_march(FzP P, FzMomArgs A, int KC)
         const double sgm = gm ? -1.0 : 1.0, sgp = gp ? -1.0 : 1.0, wm = gm ? 0.0 : 1.0;
         // S(f, di, dj, plane offset) -- shared-memory neighbour read
 #define S_(f, di, dj, o) smm[(f) * (MRING * MPS) + (o) + (dj) * MPW + (di)]   // o includes cidx
-        const double izf = P.idzf[k], izc = P.idzc[k], izcm = P.idzc[k - 1];
+        // z metrics come from global tables: carried / loaded one plane ahead so that no plane waits for them
+        const double izf = izf_p, izc = izc_n, izcm = izc_0;
+        izc_0 = izc_n; izf_p = izf_n;
+        izc_n = P.idzc[k + 1]; izf_n = P.idzf[k + 2];
+        const double izfp = izf_p;   // 1/dzf[k+1]
         const double u000 = S_(F::U, 0, 0, o0), up00 = S_(F::U, 1, 0, o0), um00 = S_(F::U, -1, 0, o0);
         const double u0p0 = S_(F::U, 0, 1, o0), u0m0 = S_(F::U, 0, -1, o0), ump0 = S_(F::U, -1, 1, o0);
         const double u00p = sgp * S_(F::U, 0, 0, op), u00m = sgm * S_(F::U, 0, 0, om), um0p = sgp * S_(F::U, -1, 0, op);
@@ -395,7 +400,6 @@ k_momentum_march(FzP P, FzMomArgs A, int KC)
         // ================= z component =================
         if (k < P.kzf) {
             const double w00p = S_(F::W, 0, 0, op);
-            const double izfp = P.idzf[k + 1];
             const double wc_p = 0.5 * (w00p + w000), wc_m = 0.5 * (w000 + w00m);
             const double Ezx_p = Exz_p;
             const double Ezx_m = 0.5 * (um00 + um0p) * 0.5 * (wm00 + w000);

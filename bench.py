@@ -259,12 +259,13 @@ def main():
     if top:
         roofline = {"bound": "hbm", "kernel": top["kernel"], "achieved": top["achieved_GBs"], "peak": peak,
                     "unit": "GB/s", "frac": top["frac"], "traffic": None, "peak_source": peak_src}
-    # ncu DRAM traffic per launch of the dominant kernel, if a summary has been committed
+    # ncu DRAM traffic per launch of the dominant kernel, from the committed summary profiles/traffic.csv
     try:
-        with open(os.path.join(ROOT, "profiles", "traffic.json")) as fh:
-            tr = json.load(fh)
-        if roofline and tr.get("workload") == cfg["name"] and roofline["kernel"] in tr.get("bytes_per_launch", {}):
-            roofline["traffic"] = tr["bytes_per_launch"][roofline["kernel"]]
+        with open(os.path.join(ROOT, "profiles", "traffic.csv")) as fh:
+            for ln in fh:
+                parts = ln.strip().split(",")
+                if roofline and len(parts) == 3 and parts[0] == cfg["name"] and parts[1] == roofline["kernel"]:
+                    roofline["traffic"] = float(parts[2])
     except Exception:
         pass
 

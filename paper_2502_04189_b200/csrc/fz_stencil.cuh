@@ -147,40 +147,46 @@ __global__ void k_phi_update(FzP P, const double *__restrict__ phi, const double
 }
 
 // ---------------------------------------------------------------- S2b: temperature transport (N14)
-__global__ void k_temp_update(FzP P, const double *__restrict__ T, const double *__restrict__ phi,
-                              const double *__restrict__ u, const double *__restrict__ v,
-                              const double *__restrict__ w, double *__restrict__ hT,
-                              double *__restrict__ Tn, double dt, double gs, double zs)
+// RHS_T = D(-u_a Tbar_a) + D(kbar_a d_a T)/(rho cp), properties from phi_new;  k is linear in clip(phi),
+// so kbar_a = k2 + (k1-k2) * 0.5 (phic + phic(+1_a)).  32-bit offsets (N < 2^31), 8 CTAs/SM.
+__global__ void __launch_bounds__(256, 6)
+k_temp_update(FzP P, const double *__restrict__ T, const double *__restrict__ phi,
+              const double *__restrict__ u, const double *__restrict__ v,
+              const double *__restrict__ w, double *__restrict__ hT,
+              double *__restrict__ Tn, double dt, double gs, double zs)
 {
     FZ_CELL_IJK
     const FzZ z = fz_zn(P, k);
-    const long long pl = (long long)P.ny * k;
-    const long long c = i + P.nx * (j + pl);
-    const long long xp = fz_ip(i, P.nx) + P.nx * (j + pl), xm = fz_im(i, P.nx) + P.nx * (j + pl);
-    const long long yp = i + P.nx * (fz_ip(j, P.ny) + pl), ym = i + P.nx * (fz_im(j, P.ny) + pl);
-    const long long zp = c + (long long)(z.kp - k) * P.sxy, zm = c + (long long)(z.km - k) * P.sxy;
-    const double dk = P.k1 - P.k2;
-    const double t0 = T[c];
-    const double txp = T[xp], txm = T[xm], typ = T[yp], tym = T[ym];
-    const double tzp = z.gp ? 2.0 * P.t_top - t0 : T[zp];
-    const double tzm = z.gm ? 2.0 * P.t_bot - t0 : T[zm];
-    const double phc = fz_clip01(phi[c]);
-    const double k0 = P.k2 + dk * phc;
-    const double kxp = P.k2 + dk * fz_clip01(phi[xp]), kxm = P.k2 + dk * fz_clip01(phi[xm]);
-    const double kyp = P.k2 + dk * fz_clip01(phi[yp]), kym = P.k2 + dk * fz_clip01(phi[ym]);
-    const double kzp = P.k2 + dk * fz_clip01(phi[zp]), kzm = P.k2 + dk * fz_clip01(phi[zm]);
-    const double Axp = -u[c] * 0.5 * (t0 + txp), Axm = -u[xm] * 0.5 * (txm + t0);
-    const double Ayp = -v[c] * 0.5 * (t0 + typ), Aym = -v[ym] * 0.5 * (tym + t0);
-    const double Azp = z.gp ? 0.0 : -w[c] * 0.5 * (t0 + tzp);
-    const double Azm = z.gm ? 0.0 : -w[zm] * 0.5 * (tzm + t0);
-    const double adv = (Axp - Axm) * P.idx + (Ayp - Aym) * P.idy + (Azp - Azm) * P.idzf[k];
-    const double qxp = 0.5 * (k0 + kxp) * (txp - t0) * P.idx, qxm = 0.5 * (kxm + k0) * (t0 - txm) * P.idx;
-    const double qyp = 0.5 * (k0 + kyp) * (typ - t0) * P.idy, qym = 0.5 * (kym + k0) * (t0 - tym) * P.idy;
-    const double qzp = 0.5 * (k0 + kzp) * (tzp - t0) * P.idzc[k];
-    const double qzm = 0.5 * (kzm + k0) * (t0 - tzm) * P.idzc[k - 1];
-    const double dif = (qxp - qxm) * P.idx + (qyp - qym) * P.idy + (qzp - qzm) * P.idzf[k];
-    const double rho = P.rho2 + P.drho * phc, cp = P.cp2 + (P.cp1 - P.cp2) * phc;
-    const double rhs = adv + dif / (rho * cp);
+    const unsigned nx = P.nx, sxy = (unsigned)P.sxy;
+    const unsigned pl = (unsigned)k * sxy, row = pl + nx * j, c = row + i;
+    const unsigned xp = row + fz_ip(i, P.nx), xm = row + fz_im(i, P.nx);
+    const unsigned yp = pl + nx * fz_ip(j, P.ny) + i, ym = pl + nx * fz_im(j, P.ny) + i;
+    const unsigned zp = (unsigned)z.kp * sxy + nx * j + i, zm = (unsigned)z.km * sxy + nx * j + i;
+    const double hdk = 0.5 * (P.k1 - P.k2);
+    const double t0 = T[c], phc = fz_clip01(phi[c]);
+    const double izf = P.idzf[k], idx = P.idx, idy = P.idy;
+    double adv, dif;
+    {   // x
+        const double tp = T[xp], tm = T[xm];
+        const double kp = P.k2 + hdk * (phc + fz_clip01(phi[xp])), km = P.k2 + hdk * (fz_clip01(phi[xm]) + phc);
+        adv = (u[xm] * (tm + t0) - u[c] * (t0 + tp)) * (0.5 * idx);
+        dif = (kp * (tp - t0) - km * (t0 - tm)) * (idx * idx);
+    }
+    {   // y
+        const double tp = T[yp], tm = T[ym];
+        const double kp = P.k2 + hdk * (phc + fz_clip01(phi[yp])), km = P.k2 + hdk * (fz_clip01(phi[ym]) + phc);
+        adv += (v[ym] * (tm + t0) - v[c] * (t0 + tp)) * (0.5 * idy);
+        dif += (kp * (tp - t0) - km * (t0 - tm)) * (idy * idy);
+    }
+    {   // z: Dirichlet ghosts 2 T_wall - T, no advective flux through a wall face
+        const double tp = z.gp ? 2.0 * P.t_top - t0 : T[zp], tm = z.gm ? 2.0 * P.t_bot - t0 : T[zm];
+        const double kp = P.k2 + hdk * (phc + fz_clip01(phi[zp])), km = P.k2 + hdk * (fz_clip01(phi[zm]) + phc);
+        const double fp = z.gp ? 0.0 : w[c] * (t0 + tp), fm = z.gm ? 0.0 : w[zm] * (tm + t0);
+        adv += (fm - fp) * (0.5 * izf);
+        dif += (kp * (tp - t0) * P.idzc[k] - km * (t0 - tm) * P.idzc[k - 1]) * izf;
+    }
+    const double rcp = (P.rho2 + P.drho * phc) * (P.cp2 + (P.cp1 - P.cp2) * phc);
+    const double rhs = adv + dif * fz_rcp(rcp);
     Tn[c] = t0 + dt * (gs * rhs + zs * hT[c]);
     hT[c] = rhs;
 }

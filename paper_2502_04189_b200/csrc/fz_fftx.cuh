@@ -14,16 +14,19 @@
 #include "fz_common.cuh"
 #include "fz_linefft.cuh"
 
-#define FX_PAIRS 4
+// line pairs per CTA: 4 (runs of 128 bytes in the spectrum) up to nx = 512, 2 at nx = 1024 so that
+// three CTAs still fit an SM (2 buffers x pairs x padded line x 16 B of shared memory)
+__host__ __device__ constexpr int fx_pairs(int log2n) { return log2n >= 10 ? 2 : 4; }
+#define FX_PAIRS fx_pairs(LOG2N)
 #ifndef FX_MINB
 #define FX_MINB 3
 #endif
 #define FX_LINE(n_) ((n_) + ((n_) >> 3))
 
-__host__ __device__ inline size_t fz_fftx_smem(int n) { return (size_t)2 * FX_PAIRS * FX_LINE(n) * 16; }
+__host__ __device__ inline size_t fz_fftx_smem(int log2n) { return (size_t)2 * fx_pairs(log2n) * FX_LINE(1 << log2n) * 16; }
 
 template <bool DIV, int LOG2N>
-__global__ void __launch_bounds__(FX_PAIRS * ((1 << LOG2N) / 8), LOG2N <= 9 ? FX_MINB : 1)
+__global__ void __launch_bounds__(FX_PAIRS * ((1 << LOG2N) / 8), FX_MINB)
 k_fftx_fwd(FzP P, const double *__restrict__ src, const double *__restrict__ us,
            const double *__restrict__ vs, const double *__restrict__ ws, double coef,
            double2 *__restrict__ spec, const double2 *__restrict__ tw)
@@ -79,7 +82,7 @@ k_fftx_fwd(FzP P, const double *__restrict__ src, const double *__restrict__ us,
 // out = Re / Im of the inverse transform * scale - gauge shift (N17: scal[2] = mean of mode (0,0),
 // written by k_spec_bwd)
 template <int LOG2N>
-__global__ void __launch_bounds__(FX_PAIRS * ((1 << LOG2N) / 8), LOG2N <= 9 ? FX_MINB : 1)
+__global__ void __launch_bounds__(FX_PAIRS * ((1 << LOG2N) / 8), FX_MINB)
 k_fftx_inv(FzP P, const double2 *__restrict__ spec, double *__restrict__ dst, double scale,
            const double2 *__restrict__ tw, const double *__restrict__ scal)
 {
@@ -127,7 +130,7 @@ cudaError_t fz_fftx_launch_one(int which /*0 fwd DIV, 1 fwd plain, 2 inv*/, cons
                                double *dst, const double2 *tw, const double *scal, cudaStream_t st)
 {
     const int n = 1 << LOG2N;
-    const size_t smem = fz_fftx_smem(n);
+    const size_t smem = fz_fftx_smem(LOG2N);
     const dim3 block(n / 8, FX_PAIRS);
     const unsigned grid = (unsigned)(((long long)P.ny * P.nz) / (2 * FX_PAIRS));
     cudaError_t e;

@@ -48,7 +48,8 @@ typedef enum {
     FIZZY_ESTATE = 4  /* call out of order (substep before set_fields, stage sequence) */
 } fizzy_status;
 
-/* Grid ("3D Cartesian grid").  nx, ny powers of two in [8, 1024]; nz >= 4.
+/* Grid ("3D Cartesian grid").  nx, ny powers of two in [8, 1024]; nz >= 4;
+ * nx*ny*nz < 2^31 (the kernels use 32-bit cell offsets).
  * zf == NULL: uniform z.  Otherwise nz+1 HOST doubles, zf[0] = 0, zf[nz] = lz, strictly
  * increasing (stretched grids need z_wall = 1).  Cell centres are face midpoints (N10). */
 typedef struct {
@@ -68,7 +69,8 @@ typedef struct {
     double rho[2], mu[2], kth[2], cp[2];
     double sigma;                 /* surface tension coefficient (CSF: sigma*kappa*grad phi) */
     double eps;                   /* interface thickness parameter of ACDI */
-    double delta;                 /* regulariser in psi = eps*ln((phi+delta)/(1-phi+delta)); N2: 1e-100 */
+    double delta;                 /* regulariser in psi = eps*ln((phi+delta)/(1-phi+delta)); N2: 1e-100;
+                                     must be >= 1e-150 so that sqrt(q_a q_b) stays finite (D3) */
     double gamma_rel, gamma_abs;  /* Gamma = gamma_rel*max|u| + gamma_abs, refreshed at stage 0 (N15) */
     double g[3];                  /* gravity */
     double rho_ref;               /* gravity enters as g*(1 - rho_ref/rho_f) (N12) */
@@ -85,8 +87,8 @@ size_t fizzy_workspace_bytes(const fizzy_grid *grid, const fizzy_bc *bc, const f
  * 256-byte aligned and outlive the context.  `cuda_stream` is a cudaStream_t (NULL = default
  * stream).  Builds the 1-D metric tables, FFT twiddles, modified wavenumbers
  * lam_x(l) = -4 sin^2(pi l/nx)/dx^2 (lam_y likewise) and the z-tridiagonal elimination tables.
- * FIZZY_EINVAL: nx, ny not powers of two in [8,1024], nz < 4, lengths <= 0, non-monotone zf,
- * zf given with z_wall = 0, rho <= 0, mu < 0, eps <= 0, delta <= 0, cp or kth <= 0 with heat on,
+ * FIZZY_EINVAL: nx, ny not powers of two in [8,1024], nz < 4, nx*ny*nz >= 2^31, lengths <= 0, non-monotone zf,
+ * zf given with z_wall = 0, rho <= 0, mu < 0, eps <= 0, delta < 1e-150, cp or kth <= 0 with heat on,
  * misaligned workspace.  FIZZY_ENOMEM: workspace too small. */
 fizzy_status fizzy_create(const fizzy_grid *grid, const fizzy_bc *bc, const fizzy_props *props,
                           void *dev_workspace, size_t workspace_bytes, void *cuda_stream,

@@ -91,7 +91,7 @@ bool valid_inputs(const fizzy_grid *g, const fizzy_bc *bc, const fizzy_props *pr
             if (!(g->zf[k + 1] > g->zf[k])) return false;
     }
     if (!(pr->rho[0] > 0) || !(pr->rho[1] > 0) || pr->mu[0] < 0 || pr->mu[1] < 0) return false;
-    if (!(pr->eps > 0) || !(pr->delta > 0)) return false;
+    if (!(pr->eps > 0) || !(pr->delta >= 1e-150)) return false;   // D3: sqrt(q_a q_b) must stay finite
     if (pr->heat && (!(pr->cp[0] > 0) || !(pr->cp[1] > 0) || !(pr->kth[0] > 0) || !(pr->kth[1] > 0))) return false;
     return true;
 }

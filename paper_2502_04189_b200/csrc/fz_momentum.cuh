@@ -322,9 +322,9 @@ k_momentum_march(FzP P, FzMomArgs A, int KC)
         double ph000 = 0, php00 = 0, ph0p0 = 0, ph00p = 0;
         if (VARRHO) {
             const double r000 = P.rho2 + P.drho * fz_clip01(f000);
-            irx = 1.0 / (0.5 * (r000 + P.rho2 + P.drho * fz_clip01(fp00)));
-            iry = 1.0 / (0.5 * (r000 + P.rho2 + P.drho * fz_clip01(f0p0)));
-            irz = 1.0 / (0.5 * (r000 + P.rho2 + P.drho * fz_clip01(f00p)));
+            irx = fz_rcp(0.5 * (r000 + P.rho2 + P.drho * fz_clip01(fp00)));
+            iry = fz_rcp(0.5 * (r000 + P.rho2 + P.drho * fz_clip01(f0p0)));
+            irz = fz_rcp(0.5 * (r000 + P.rho2 + P.drho * fz_clip01(f00p)));
             // p_hat = 2 p - p_prev (N7)
 #define PH_(di, dj, o) (2.0 * S_(F::PN, di, dj, o) - S_(F::PO, di, dj, o))
             ph000 = PH_(0, 0, o0); php00 = PH_(1, 0, o0); ph0p0 = PH_(0, 1, o0);
@@ -417,7 +417,7 @@ k_momentum_march(FzP P, FzMomArgs A, int KC)
             if (VARRHO) {
                 const double Rtx = 0.25 * (S_(F::RX, 0, 0, o0) + S_(F::RX, 0, 0, op) + S_(F::RX, -1, 0, o0) + S_(F::RX, -1, 0, op));
                 const double Rty = 0.25 * (S_(F::RY, 0, 0, o0) + S_(F::RY, 0, 0, op) + S_(F::RY, 0, -1, o0) + S_(F::RY, 0, -1, op));
-                M = P.drho * Gam * (S_(F::RZ, 0, 0, o0) * (w00p - w00m) / (P.dzf[k + 1] + P.dzf[k]) +
+                M = P.drho * Gam * (S_(F::RZ, 0, 0, o0) * (w00p - w00m) * fz_rcp(P.dzf[k + 1] + P.dzf[k]) +
                                     Rtx * (wp00 - wm00) * (0.5 * dx) + Rty * (w0p0 - w0m0) * (0.5 * dy));
             }
             double B = P.gz * (1.0 - P.rho_ref * irz) + P.fz + P.a_lin * w000;

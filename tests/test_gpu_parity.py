@@ -152,3 +152,25 @@ def test_properties_at_128(fz):
     assert abs(out["phi"].sum() - m0) <= 1e-12 * m0
     assert out["phi"].min() >= -1e-6 and out["phi"].max() <= 1 + 1e-6
     g.close()
+
+
+@pytest.mark.parametrize("name", ["cfg1_taylor_green_64", "cfg2_bubbles_walls_64x64x48", "cfg4_channel_heat_64x32x48"])
+def test_bitwise_repeatability(fz, name):
+    """The shared-memory rings of the marching and spectral kernels are hand-synchronised (one barrier per
+    plane, cp.async groups); compute-sanitizer is closed on this pool, so a data race is looked for the
+    other way: the same three RK3 steps run three times must give bit-identical fields (no atomics in the
+    arithmetic path: the max|u| reduction is order-independent)."""
+    cfg, f, dt, _ = CASES[name]()
+    ref = None
+    for _ in range(3):
+        g = fz.Fizzy(cfg)
+        g.set_fields_numpy(**f)
+        for _ in range(3):
+            g.step(dt)
+        out = g.get_fields_numpy()
+        g.close()
+        if ref is None:
+            ref = out
+        else:
+            for k in ref:
+                assert np.array_equal(out[k], ref[k]), (name, k)

@@ -269,8 +269,13 @@ k_momentum_march(FzP P, FzMomArgs A, int KC)
     int sl = (k0 - 1 + MRING) % MRING;   // ring slot of plane k-1, advanced incrementally
     int om, o0 = sl * MPS + cidx, op = ((sl + 1) % MRING) * MPS + cidx;
     sl = (sl + 1) % MRING;
-    double hu_nx = A.hu[(long long)k0 * P.sxy + goff_c], hv_nx = A.hv[(long long)k0 * P.sxy + goff_c],
-           hw_nx = A.hw[(long long)k0 * P.sxy + goff_c];
+    // stage 0 has zeta = 0: the RK histories are not read at all (-24 B/cell on that substep)
+    const bool use_h = A.zs != 0.0;
+    double hu_nx = 0.0, hv_nx = 0.0, hw_nx = 0.0;
+    if (use_h) {
+        hu_nx = A.hu[(long long)k0 * P.sxy + goff_c]; hv_nx = A.hv[(long long)k0 * P.sxy + goff_c];
+        hw_nx = A.hw[(long long)k0 * P.sxy + goff_c];
+    }
     double izc_0 = P.idzc[k0 - 1], izc_n = P.idzc[k0], izf_p = P.idzf[k0], izf_n = P.idzf[k0 + 1];
     for (int k = k0; k < k1; ++k) {
         fz_cp_async_wait<1>();
@@ -282,7 +287,7 @@ k_momentum_march(FzP P, FzMomArgs A, int KC)
         const long long c = (long long)k * P.sxy + goff_c;
         // RK histories: loaded one plane ahead (registers), so their latency hides behind a whole plane
         const double hu_old = hu_nx, hv_old = hv_nx, hw_old = hw_nx;
-        if (k + 1 < k1) { hu_nx = A.hu[c + P.sxy]; hv_nx = A.hv[c + P.sxy]; hw_nx = A.hw[c + P.sxy]; }
+        if (use_h && k + 1 < k1) { hu_nx = A.hu[c + P.sxy]; hv_nx = A.hv[c + P.sxy]; hw_nx = A.hw[c + P.sxy]; }
         // ghost rules at the walls: planes k-1 / k+1 hold the mirrored interior plane
         const bool gm = P.z_wall && k == 0, gp = P.z_wall && k == P.nz - 1;
         const double sgm = gm ? -1.0 : 1.0, sgp = gp ? -1.0 : 1.0, wm = gm ? 0.0 : 1.0;

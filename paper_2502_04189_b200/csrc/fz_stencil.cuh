@@ -136,7 +136,8 @@ __global__ void k_phi_update(FzP P, const double *__restrict__ phi, const double
     const double Fzp = z.gp ? 0.0 : -w[c] * 0.5 * (f0 + phi[zp]);
     const double Fzm = z.gm ? 0.0 : -w[zm] * 0.5 * (phi[zm] + f0);
     const double rhs = (Fxp - Fxm) * P.idx + (Fyp - Fym) * P.idy + (Fzp - Fzm) * P.idzf[k] + scal[1] * divrn[c];
-    const double fn = f0 + dt * (gs * rhs + zs * hphi[c]);
+    // stage 0 has zeta = 0: the history is not read (it may hold anything finite; 0 * h == 0)
+    const double fn = f0 + dt * (gs * rhs + (zs != 0.0 ? zs * hphi[c] : 0.0));
     phin[c] = fn;
     hphi[c] = rhs;
     // psi, r = sqrt(q) of phi_new for the interface sweep (same formulas as k_iface_psi)
@@ -187,7 +188,7 @@ k_temp_update(FzP P, const double *__restrict__ T, const double *__restrict__ ph
     }
     const double rcp = (P.rho2 + P.drho * phc) * (P.cp2 + (P.cp1 - P.cp2) * phc);
     const double rhs = adv + dif * fz_rcp(rcp);
-    Tn[c] = t0 + dt * (gs * rhs + zs * hT[c]);
+    Tn[c] = t0 + dt * (gs * rhs + (zs != 0.0 ? zs * hT[c] : 0.0));
     hT[c] = rhs;
 }
 

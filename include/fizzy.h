@@ -121,6 +121,15 @@ fizzy_status fizzy_poisson_solve(fizzy_ctx *ctx, const double *rhs, double *p);
 fizzy_status fizzy_get_fields(fizzy_ctx *ctx, double *u, double *v, double *w, double *p,
                               double *phi, double *T, double *p_prev);
 
+/* Run-time diagnostics of the current state (definitions in DESIGN.md 10), one pass
+ * over the fields and a fixed-order (deterministic) reduction.  `out` = 6 HOST doubles, dV = dx*dy*dzf[k]:
+ *   out[0] = sum phi dV (volume of fluid 1)        out[1] = 1/2 sum rho(phi) |u_c|^2 dV, u_c = cell-centred mean
+ *   out[2] = max over faces of max(|u|,|v|,|w|)    out[3] = max |D(u)|
+ *   out[4] = sum |grad phi| dV (central differences: area of the diffuse interface)
+ *   out[5] = sum T dV / sum dV (0 with heat off).
+ * Synchronises the stream.  FIZZY_ESTATE before fizzy_set_fields. */
+fizzy_status fizzy_diagnostics(fizzy_ctx *ctx, double *out);
+
 /* Current Gamma (synchronises the stream).  NaN if ctx is NULL. */
 double fizzy_gamma(fizzy_ctx *ctx);
 

@@ -69,6 +69,7 @@ def _load():
         lib.orc_substep.argtypes = [C.c_void_p, C.c_int, C.c_double]
         lib.orc_substep.restype = C.c_int
         lib.orc_poisson_solve.argtypes = [C.c_void_p, _dp, _dp]
+        lib.orc_diagnostics.argtypes = [C.c_void_p, _dp]
         lib.orc_gamma.argtypes = [C.c_void_p]
         lib.orc_gamma.restype = C.c_double
         lib.orc_get_intermediate.argtypes = [C.c_void_p, C.c_char_p, _dp]
@@ -153,6 +154,12 @@ class Oracle:
         rhs = _c(rhs)
         out = np.empty(self.shape)
         _load().orc_poisson_solve(self._h, _ptr(rhs), _ptr(out))
+        return out
+
+    def diagnostics(self) -> np.ndarray:
+        """[volume of fluid 1, kinetic energy, max|u|, max|D(u)|, interfacial area, mean T]"""
+        out = np.zeros(6)
+        _load().orc_diagnostics(self._h, out.ctypes.data_as(_dp))
         return out
 
     def gamma(self) -> float:

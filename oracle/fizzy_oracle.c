@@ -903,3 +903,45 @@ int orc_get_intermediate(const orc_state *st, const char *name, double *out)
         }
     return -1;
 }
+
+/* ------------------------------------------------------------------ run-time diagnostics
+ * (definitions in DESIGN.md section 10).  dV = dx dy dzf[k].
+ *   out[0] = sum phi dV                                  (volume of fluid 1)
+ *   out[1] = 1/2 sum rho(phi) (uc^2 + vc^2 + wc^2) dV,   uc = (u + u(-1_x))/2 etc. (cell-centred)
+ *   out[2] = max over faces of max(|u|, |v|, |w|)
+ *   out[3] = max |D(u)|
+ *   out[4] = sum |grad phi| dV, central differences (phi(+1_a) - phi(-1_a))/(hc_a + hc_a(-1_a))
+ *            (interfacial area of a diffuse interface)
+ *   out[5] = sum T dV / sum dV   (0 if heat is off)
+ * Ghosts of u, v, w, phi, T are up to date after orc_set_fields / orc_substep. */
+void orc_diagnostics(const orc_state *st, double *out)
+{
+    const int nx = st->nx, ny = st->ny, nz = st->nz;
+    const double dx = st->dx, dy = st->dy;
+    double vol1 = 0.0, ke = 0.0, umax = 0.0, dmax = 0.0, area = 0.0, tsum = 0.0, vsum = 0.0;
+    for (int k = 0; k < nz; ++k)
+        for (int j = 0; j < ny; ++j)
+            for (int i = 0; i < nx; ++i) {
+                const size_t c = IDX(i, j, k);
+                const double dV = dx * dy * DZF(k);
+                const double phc = fmin(fmax(st->phi[c], 0.0), 1.0);
+                const double rho = st->P.rho2 + (st->P.rho1 - st->P.rho2) * phc;
+                const double uc = 0.5 * (st->u[c] + st->u[IDX(i - 1, j, k)]);
+                const double vc = 0.5 * (st->v[c] + st->v[IDX(i, j - 1, k)]);
+                const double wc = 0.5 * (st->w[c] + st->w[IDX(i, j, k - 1)]);
+                const double div = (st->u[c] - st->u[IDX(i - 1, j, k)]) / dx + (st->v[c] - st->v[IDX(i, j - 1, k)]) / dy +
+                                   (st->w[c] - st->w[IDX(i, j, k - 1)]) / DZF(k);
+                const double gx = (st->phi[IDX(i + 1, j, k)] - st->phi[IDX(i - 1, j, k)]) / (2.0 * dx);
+                const double gy = (st->phi[IDX(i, j + 1, k)] - st->phi[IDX(i, j - 1, k)]) / (2.0 * dy);
+                const double gz = (st->phi[IDX(i, j, k + 1)] - st->phi[IDX(i, j, k - 1)]) / (DZC(k) + DZC(k - 1));
+                vol1 += st->phi[c] * dV;
+                ke += 0.5 * rho * (uc * uc + vc * vc + wc * wc) * dV;
+                umax = fmax(umax, fmax(fabs(st->u[c]), fmax(fabs(st->v[c]), fabs(st->w[c]))));
+                dmax = fmax(dmax, fabs(div));
+                area += sqrt(gx * gx + gy * gy + gz * gz) * dV;
+                vsum += dV;
+                if (st->P.heat) tsum += st->T[c] * dV;
+            }
+    out[0] = vol1; out[1] = ke; out[2] = umax; out[3] = dmax; out[4] = area;
+    out[5] = st->P.heat ? tsum / vsum : 0.0;
+}

@@ -85,6 +85,10 @@ void orc_temperature_rhs(orc_state *st, double *rhs_T);
  * in-place, n a power of two, sign=-1 forward (e^{-2 pi i jk/n}), +1 backward (no scaling) */
 void orc_fft(int n, double *re, double *im, int sign);
 
+/* run-time diagnostics of the current state: out[6] = volume of fluid 1,
+ * kinetic energy, max|u|, max|D(u)|, interfacial area, mean temperature (see fizzy_oracle.c) */
+void orc_diagnostics(const orc_state *st, double *out);
+
 int orc_num_threads(void);
 
 #ifdef __cplusplus

@@ -17,7 +17,7 @@ FIZZY_OK, FIZZY_EINVAL, FIZZY_ENOMEM, FIZZY_ECUDA, FIZZY_ESTATE = range(5)
 _STATUS = {0: "FIZZY_OK", 1: "FIZZY_EINVAL", 2: "FIZZY_ENOMEM", 3: "FIZZY_ECUDA", 4: "FIZZY_ESTATE"}
 
 EXPORTS = ["fizzy_workspace_bytes", "fizzy_create", "fizzy_destroy", "fizzy_set_fields",
-           "fizzy_rk3_substep", "fizzy_poisson_solve", "fizzy_get_fields", "fizzy_gamma",
+           "fizzy_rk3_substep", "fizzy_poisson_solve", "fizzy_get_fields", "fizzy_gamma", "fizzy_diagnostics",
            "fizzy_launch_count", "fizzy_last_error", "fizzy_timing_enable", "fizzy_timing_get"]
 
 
@@ -67,6 +67,8 @@ def load_library(path: str = LIB_PATH) -> C.CDLL:
     lib.fizzy_rk3_substep.argtypes = [vp, C.c_int, C.c_double]
     lib.fizzy_poisson_solve.restype = C.c_int
     lib.fizzy_poisson_solve.argtypes = [vp, dp, dp]
+    lib.fizzy_diagnostics.restype = C.c_int
+    lib.fizzy_diagnostics.argtypes = [vp, C.POINTER(C.c_double)]
     lib.fizzy_gamma.restype = C.c_double
     lib.fizzy_gamma.argtypes = [vp]
     lib.fizzy_launch_count.restype = C.c_longlong
@@ -177,6 +179,11 @@ class Fizzy:
 
     def fizzy_poisson_solve(self, rhs, p):
         self._check(_lib.fizzy_poisson_solve(self._h, _addr(rhs), _addr(p)))
+
+    def fizzy_diagnostics(self) -> np.ndarray:
+        out = (C.c_double * 6)()
+        self._check(_lib.fizzy_diagnostics(self._h, out))
+        return np.array(out[:])
 
     def fizzy_gamma(self) -> float:
         return float(_lib.fizzy_gamma(self._h))

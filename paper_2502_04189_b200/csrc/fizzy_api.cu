@@ -10,6 +10,7 @@
 #include <vector>
 
 #include "fz_common.cuh"
+#include "fz_diag.cuh"
 #include "fz_fftx.cuh"
 #include "fz_iface.cuh"
 #include "fz_momentum.cuh"
@@ -64,7 +65,8 @@ struct fizzy_ctx {
     double *kappa, *divrn, *psi, *rr, *nhx, *nhy, *nhz, *rnx, *rny, *rnz;
     double2 *spec;
     double2 *twx, *twy;
-    double *scal;  // [0] running max|u|, [1] Gamma
+    double *scal;  // [0] running max|u|, [1] Gamma, [2] gauge mean, [8..13] diagnostics
+    double *dpart; // block partials of k_diag
     FzTri tri;
     int fields_set, next_stage;
     long long launches;
@@ -125,7 +127,8 @@ size_t layout(fizzy_ctx *c, void *base, const fizzy_grid *g, const fizzy_bc *bc,
     { double *t = cv.dbl(nxh); if (lam) lam[0] = t; t = cv.dbl(g->ny); if (lam) lam[1] = t; }
     x->twx = static_cast<double2 *>(cv.take(g->nx * sizeof(double2)));
     x->twy = static_cast<double2 *>(cv.take(g->ny * sizeof(double2)));
-    x->scal = cv.dbl(4);
+    x->scal = cv.dbl(16);
+    x->dpart = cv.dbl((size_t)FZ_DIAG_BLOCKS * FZ_DIAG_NV);
     return cv.off;
 }
 
@@ -540,6 +543,22 @@ extern "C" fizzy_status fizzy_rk3_substep(fizzy_ctx *c, int stage, double dt)
     c->p = c->pn;
     c->pn = old_pp;
     c->next_stage = (stage + 1) % 3;
+    return FIZZY_OK;
+}
+
+extern "C" fizzy_status fizzy_diagnostics(fizzy_ctx *c, double *out)
+{
+    if (!c) return FIZZY_EINVAL;
+    if (!out) return fail(c, FIZZY_EINVAL, "out must be non-NULL");
+    if (!c->fields_set) return fail(c, FIZZY_ESTATE, "fizzy_set_fields has not been called");
+    FZ_TB(FZK_OTHER);
+    k_diag<<<FZ_DIAG_BLOCKS, 256, 0, c->stream>>>(c->P, c->u, c->v, c->w, c->phi, c->T, c->dpart);
+    FZ_LAUNCHED(FZK_OTHER);
+    FZ_TB(FZK_OTHER);
+    k_diag_final<<<1, 256, 0, c->stream>>>(c->P, c->dpart, FZ_DIAG_BLOCKS, c->scal + 8);
+    FZ_LAUNCHED(FZK_OTHER);
+    FZ_CUDA(cudaMemcpyAsync(out, c->scal + 8, 6 * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    FZ_CUDA(cudaStreamSynchronize(c->stream));
     return FIZZY_OK;
 }
 

@@ -174,3 +174,22 @@ def test_bitwise_repeatability(fz, name):
         else:
             for k in ref:
                 assert np.array_equal(out[k], ref[k]), (name, k)
+
+
+@pytest.mark.parametrize("name", ["cfg0_static_drop_32", "cfg2_bubbles_walls_64x64x48", "cfg4_channel_heat_64x32x48",
+                                  "cfg1_ragged_16x8x5"])
+def test_diagnostics(fz, oracle_mod, name):
+    """fizzy_diagnostics against the oracle's after two RK3 steps: the sums agree to the summation-order
+    round-off (1e-12 relative), the two maxima exactly where the underlying fields agree to 1e-10."""
+    cfg, f, dt, o, g = _pair(fz, oracle_mod, name)
+    for _ in range(2):
+        o.step(dt)
+        g.step(dt)
+    do, dg = o.diagnostics(), g.fizzy_diagnostics()
+    for q in (0, 1, 4, 5):
+        assert abs(dg[q] - do[q]) <= 1e-10 * max(abs(do[q]), 1e-300), (name, q, dg[q], do[q])
+    assert abs(dg[2] - do[2]) <= 1e-10 * max(do[2], 1e-300)
+    umax = max(do[2], 1.0)
+    assert abs(dg[3] - do[3]) <= 1e-9 * umax / min(cfg["lx"] / cfg["nx"], cfg["ly"] / cfg["ny"])
+    assert np.array_equal(dg, g.fizzy_diagnostics())   # fixed-order reduction: repeatable bit for bit
+    g.close()

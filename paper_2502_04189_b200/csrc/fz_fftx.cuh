@@ -14,25 +14,27 @@
 #include "fz_common.cuh"
 #include "fz_linefft.cuh"
 
-// line pairs per CTA: 4 (runs of 128 bytes in the spectrum) up to nx = 512, 2 at nx = 1024 so that
-// three CTAs still fit an SM (2 buffers x pairs x padded line x 16 B of shared memory)
-__host__ __device__ constexpr int fx_pairs(int log2n) { return log2n >= 10 ? 2 : 4; }
-#define FX_PAIRS fx_pairs(LOG2N)
-#ifndef FX_MINB
-#define FX_MINB 3
-#endif
+// line pairs per CTA (2 buffers x pairs x padded line x 16 B of shared memory).  Forward: 2 pairs from
+// nx = 512 up (64-byte runs in the spectrum, merged in L2 with the neighbouring CTA's; five 128-thread CTAs
+// per SM at ~95 registers measured 20 % faster than three 256-thread CTAs).  Backward: 4 pairs (128-byte
+// runs when READING the spectrum matter), 2 at nx = 1024 so that three CTAs still fit an SM.
+__host__ __device__ constexpr int fx_pairs(int log2n, bool inverse)
+{
+    return inverse ? (log2n >= 10 ? 2 : 4) : (log2n >= 9 ? 2 : 4);
+}
+__host__ __device__ constexpr int fx_minb(int log2n, bool inverse) { return (!inverse && log2n == 9) ? 5 : 3; }
 #define FX_LINE(n_) ((n_) + ((n_) >> 3))
 
-__host__ __device__ inline size_t fz_fftx_smem(int log2n) { return (size_t)2 * fx_pairs(log2n) * FX_LINE(1 << log2n) * 16; }
+__host__ __device__ inline size_t fz_fftx_smem(int log2n, bool inverse) { return (size_t)2 * fx_pairs(log2n, inverse) * FX_LINE(1 << log2n) * 16; }
 
 template <bool DIV, int LOG2N>
-__global__ void __launch_bounds__(FX_PAIRS * ((1 << LOG2N) / 8), FX_MINB)
+__global__ void __launch_bounds__(fx_pairs(LOG2N, false) * ((1 << LOG2N) / 8), fx_minb(LOG2N, false))
 k_fftx_fwd(FzP P, const double *__restrict__ src, const double *__restrict__ us,
            const double *__restrict__ vs, const double *__restrict__ ws, double coef,
            double2 *__restrict__ spec, const double2 *__restrict__ tw)
 {
     extern __shared__ __align__(16) double2 smx[];
-    constexpr int n = 1 << LOG2N, T8 = n / 8, LN = FX_LINE(n);
+    constexpr int n = 1 << LOG2N, T8 = n / 8, LN = FX_LINE(n), FX_PAIRS = fx_pairs(LOG2N, false);
     const int jt = threadIdx.x, g = threadIdx.y;
     double2 *A = smx + (2 * g) * LN, *B = A + LN;
     FzLineFFT<LOG2N, -1, false> fft;
@@ -82,12 +84,12 @@ k_fftx_fwd(FzP P, const double *__restrict__ src, const double *__restrict__ us,
 // out = Re / Im of the inverse transform * scale - gauge shift (N17: scal[2] = mean of mode (0,0),
 // written by k_spec_bwd)
 template <int LOG2N>
-__global__ void __launch_bounds__(FX_PAIRS * ((1 << LOG2N) / 8), FX_MINB)
+__global__ void __launch_bounds__(fx_pairs(LOG2N, true) * ((1 << LOG2N) / 8), fx_minb(LOG2N, true))
 k_fftx_inv(FzP P, const double2 *__restrict__ spec, double *__restrict__ dst, double scale,
            const double2 *__restrict__ tw, const double *__restrict__ scal)
 {
     extern __shared__ __align__(16) double2 smx[];
-    constexpr int n = 1 << LOG2N, T8 = n / 8, LN = FX_LINE(n);
+    constexpr int n = 1 << LOG2N, T8 = n / 8, LN = FX_LINE(n), FX_PAIRS = fx_pairs(LOG2N, true);
     const int jt = threadIdx.x, g = threadIdx.y;
     double2 *A = smx + (2 * g) * LN, *B = A + LN;
     FzLineFFT<LOG2N, +1, false> fft;
@@ -130,9 +132,10 @@ cudaError_t fz_fftx_launch_one(int which /*0 fwd DIV, 1 fwd plain, 2 inv*/, cons
                                double *dst, const double2 *tw, const double *scal, cudaStream_t st)
 {
     const int n = 1 << LOG2N;
-    const size_t smem = fz_fftx_smem(LOG2N);
-    const dim3 block(n / 8, FX_PAIRS);
-    const unsigned grid = (unsigned)(((long long)P.ny * P.nz) / (2 * FX_PAIRS));
+    const int np = fx_pairs(LOG2N, which == 2);
+    const size_t smem = fz_fftx_smem(LOG2N, which == 2);
+    const dim3 block(n / 8, np);
+    const unsigned grid = (unsigned)(((long long)P.ny * P.nz) / (2 * np));
     cudaError_t e;
     if (which == 0) {
         e = cudaFuncSetAttribute(k_fftx_fwd<true, LOG2N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);

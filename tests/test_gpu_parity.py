@@ -28,10 +28,20 @@ CASES = {
     # maximum transform lengths (1024 = 8*8*8*2: radix-8 passes + the radix-2 remainder pass)
     "cfg1_nx1024": lambda: W.make(1, grid=(1024, 16, 8), ndrops=1),
     "cfg2_ny1024_walls": lambda: W.make(2, grid=(32, 1024, 8), ndrops=1, radius=0.2),
+    # the same maximum lengths on non-degenerate grids: config 5's box and physics (heat, rho ratio 10,
+    # stretched walls) with its nx = 1024; walls + rho ratio 1000 with ny = 1024
+    "cfg4_nx1024_64x64": lambda: W.make(4, grid=(1024, 64, 64), ndrops=4, radius=0.25),
+    "cfg2_ny1024_64x32": lambda: W.make(2, grid=(64, 1024, 32), ndrops=2, radius=0.15),
 }
 
 
-MAXLEN = ("cfg1_nx1024", "cfg2_ny1024_walls")
+
+
+# nx = 1024 on a 1024 x 16 x 8 grid of the 2 pi box has dx/dz = 1/128 and max|w| = 1.4e-3 max|u|: there the
+# per-field norm of w divides a round-off of the size seen in u, v by a tiny max|w|.  For this one case the
+# velocity components are normalised by max(|u|,|v|,|w|) (measured on the B200: w 4.2e-8 per-field = 6e-11
+# of max|u| at stage 2; the same 1024-point transform passes per field on cfg4_nx1024_64x64)
+DEGENERATE = ("cfg1_nx1024",)
 
 
 def field_error(a, b):
@@ -63,15 +73,17 @@ def _pair(fz, oracle_mod, name):
 def test_one_substep_each_stage(fz, oracle_mod, name):
     """After each of the first three substeps every field matches the oracle to 1e-10."""
     cfg, f, dt, o, g = _pair(fz, oracle_mod, name)
-    # the two maximum-length cases sit on extremely anisotropic grids (dx/dz = 1/128) where w is three
-    # orders below u: they are held to the stated bar (one substep), not to three
-    for stage in range(1 if name in MAXLEN else 3):
+    for stage in range(3):
         o.substep(stage, dt)
         g.fizzy_rk3_substep(stage, dt)
         fo, fg = o.get_fields(), g.get_fields_numpy()
+        vmax = max(np.abs(fo[k]).max() for k in "uvw")
         for k in fo:
             assert np.isfinite(fg[k]).all(), (name, stage, k)
-            assert field_error(fg[k], fo[k]) <= TOL_SUBSTEP, (name, stage, k, field_error(fg[k], fo[k]))
+            e = field_error(fg[k], fo[k])
+            if name in DEGENERATE and k in "uvw":
+                e = np.abs(fg[k] - fo[k]).max() / vmax
+            assert e <= TOL_SUBSTEP, (name, stage, k, e)
         assert abs(g.fizzy_gamma() - o.gamma()) <= 1e-12 * max(1.0, abs(o.gamma()))
     g.close()
 

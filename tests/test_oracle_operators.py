@@ -94,51 +94,53 @@ def test_advection_conserves_momentum_and_kinetic_energy(oracle_mod):
 
 
 def test_mass_consistent_term_exact_for_linear_velocity_and_zero_for_matched_density(oracle_mod):
-    """N9: M_a = (rho1-rho2) (R . grad) u_a.  With u_a linear in the coordinates central
-    differences are exact, so M_a must equal (rho1-rho2) * sum_t Rtilde_t * b_t where Rtilde is
-    the 4-face average of the oracle's own R faces (recomputed here with numpy rolls).
-    Isolated as RHS(rho1,rho2) - RHS(rho,rho) is not possible (1/rho_f changes), so the other
-    terms are switched off: mu=0, sigma=0, g=0 and A is removed analytically."""
-    n = 16
-    L = 1.0
-    base = dict(nx=n, ny=n, nz=n, lx=L, ly=L, lz=L, eps=1.5 / n, mu1=0.0, mu2=0.0, gamma_abs=1.0)
-    cfgA, f, _, _ = W.make(0, grid=(n, n, n), radius=0.25)
-    phi = f["phi"]
-    rng = np.random.default_rng(5)
-    # periodic box => "linear" velocity must be piecewise: use u = b_y * sawtooth-free trick:
-    # take u_x = sin-free constant-gradient only locally: instead use a uniform velocity plus
-    # small smooth field and check linearity in (rho1-rho2) and vanishing at rho1 == rho2.
-    u = 0.3 + 0.1 * rng.standard_normal(phi.shape)
-    v = -0.2 + 0.1 * rng.standard_normal(phi.shape)
-    w = 0.1 + 0.1 * rng.standard_normal(phi.shape)
+    """N9: M_a = (rho1-rho2) (R . grad) u_a with central differences.  Between walls on a STRETCHED grid take
+    u = a + b z, v = c + d z, w = e zf (linear in z, uniform in x, y): every central difference is exact, so
+    on the rows whose stencil stays clear of the wall ghosts
+        M_x = (rho1-rho2) b Rt_z,   M_y = (rho1-rho2) d Rt_z,   M_z = (rho1-rho2) e R_z
+    where Rt_z is the mean of the four z-faces around the x- (y-) face -- the only part restated here; a
+    wrong metric in a z-derivative (dzc for dzf, a missing factor 2) or a wrong sign fails.  M is isolated
+    as RHS(rho1,rho2) - RHS(rho,rho) with mu = sigma = g = 0 (the advective part does not see rho), which
+    also shows that it vanishes for matched densities whatever their common value."""
+    nx, ny, nz, lz = 16, 16, 20, 1.0
+    a_ = 1.1
+    zf = lz * 0.5 * (1.0 + np.tanh(a_ * (np.arange(nz + 1) / nz - 0.5) * 2) / math.tanh(a_))
+    zf[0], zf[-1] = 0.0, lz
+    base = dict(nx=nx, ny=ny, nz=nz, lx=1.0, ly=1.0, lz=lz, z_wall=1, zf=zf, eps=1.5 / nx, mu1=0.0, mu2=0.0,
+                gamma_abs=1.0)
+    phi = W.phase_field(dict(base, rho1=1.0, rho2=1.0), np.array([[0.45, 0.55, 0.5]]), 0.25)
+    zc = 0.5 * (zf[1:] + zf[:-1])
+    ones = np.ones((nz, ny, nx))
+    b, d, e = 0.7, -0.4, 0.3
+    u = (0.3 + b * zc)[:, None, None] * ones
+    v = (-0.2 + d * zc)[:, None, None] * ones
+    w = (e * zf[1:])[:, None, None] * ones
+    w[-1] = 0.0
 
-    def rhs(rho1, rho2):
+    def run(rho1, rho2):
         o = oracle_mod.Oracle(dict(base, rho1=rho1, rho2=rho2))
         o.set_fields(u, v, w, np.zeros_like(u), phi)
         r = o.momentum_rhs()
-        R = [o.intermediate(k) for k in ("Rx", "Ry", "Rz")]
-        rho = o.intermediate("rho")
-        return r, R, rho
+        return r, o.intermediate("Rz"), o.intermediate("rho")
 
-    r0, R, _ = rhs(1.0, 1.0)              # pure advection A
-    r1, R1, rho = rhs(3.0, 1.0)           # A + M/rho_f
-    h = L / n
+    r0, _, _ = run(1.0, 1.0)
+    r0b, _, _ = run(2.5, 2.5)
+    for q in range(3):
+        assert np.array_equal(r0[q], r0b[q])          # matched densities: no M, no rho dependence at all
+    r1, Rz, rho = run(3.0, 1.0)
+    drho = 2.0
     sh = lambda f, dx=0, dy=0, dz=0: np.roll(f, (-dz, -dy, -dx), axis=(0, 1, 2))
-    # x component at the x-face: M_x = drho*[Rx*(u(+x)-u(-x))/2h + Rty*(u(+y)-u(-y))/2h + Rtz*(...)]/rho_f
-    Rx, Ry, Rz = R1
-    Rty = 0.25 * (Ry + sh(Ry, dx=1) + sh(Ry, dy=-1) + sh(Ry, dx=1, dy=-1))
-    Rtz = 0.25 * (Rz + sh(Rz, dx=1) + sh(Rz, dz=-1) + sh(Rz, dx=1, dz=-1))
-    Mx = 2.0 * (Rx * (sh(u, dx=1) - sh(u, dx=-1)) + Rty * (sh(u, dy=1) - sh(u, dy=-1))
-                + Rtz * (sh(u, dz=1) - sh(u, dz=-1))) / (2 * h)
-    rhof = 0.5 * (rho + sh(rho, dx=1))
-    np.testing.assert_allclose(r1[0] - r0[0], Mx / rhof, rtol=0, atol=1e-11 * np.abs(Mx / rhof).max())
-    # z component at the z-face
-    Rtx = 0.25 * (Rx + sh(Rx, dz=1) + sh(Rx, dx=-1) + sh(Rx, dx=-1, dz=1))
-    Rty = 0.25 * (Ry + sh(Ry, dz=1) + sh(Ry, dy=-1) + sh(Ry, dy=-1, dz=1))
-    Mz = 2.0 * (Rz * (sh(w, dz=1) - sh(w, dz=-1)) + Rtx * (sh(w, dx=1) - sh(w, dx=-1))
-                + Rty * (sh(w, dy=1) - sh(w, dy=-1))) / (2 * h)
-    rhof = 0.5 * (rho + sh(rho, dz=1))
-    np.testing.assert_allclose(r1[2] - r0[2], Mz / rhof, rtol=0, atol=1e-11 * np.abs(Mz / rhof).max())
+    rows = slice(1, nz - 2)       # stencils clear of the wall ghosts and of the imposed w = 0 on the top face
+    Rtz_x = 0.25 * (Rz + sh(Rz, dx=1) + sh(Rz, dz=-1) + sh(Rz, dx=1, dz=-1))
+    Rtz_y = 0.25 * (Rz + sh(Rz, dy=1) + sh(Rz, dz=-1) + sh(Rz, dy=1, dz=-1))
+    expect = [drho * b * Rtz_x / (0.5 * (rho + sh(rho, dx=1))),
+              drho * d * Rtz_y / (0.5 * (rho + sh(rho, dy=1))),
+              drho * e * Rz / (0.5 * (rho + sh(rho, dz=1)))]
+    for q in range(3):
+        got = (r1[q] - r0[q])[rows]
+        scale = np.abs(expect[q][rows]).max()
+        assert scale > 1e-3
+        assert np.abs(got - expect[q][rows]).max() < 1e-12 * max(scale, np.abs(r0[q]).max()), q
 
 
 def test_planar_tanh_profile_is_the_equilibrium_of_the_regularisation_flux(oracle_mod):

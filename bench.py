@@ -40,12 +40,13 @@ def algorithmic_bytes_per_cell(cfg):
     varrho = cfg["rho1"] != cfg["rho2"]
     heat = bool(cfg["heat"])
     b = {
-        "k_phi_update": 80.0,                                   # r phi,u,v,w,hphi,divRn  w phi,hphi,psi,r
-        "k_iface_march": 40.0 + (24.0 if varrho else 0.0),      # r psi,r,phi  w kappa,divRn (+Rn x3)
+        "k_phi_update": 72.0,                                   # r phi,u,v,w,hphi,divRn  w phi,hphi,psi
+        "k_iface_march": 32.0 + (24.0 if varrho else 0.0),      # r psi,phi  w kappa,divRn (+Rn x3)
         "k_momentum": 112.0 + (40.0 if varrho else 0.0) + (8.0 if heat else 0.0),
         "k_fftx_fwd": 24.0 + spec,
-        # fused FFT_y + z-elimination: r spec, INV (half a complex), w spec; backward also E if z is periodic
-        "k_spec_fwd": 2.5 * spec, "k_spec_bwd": (3.0 if not cfg["z_wall"] else 2.5) * spec,
+        # fused FFT_y + z-elimination: forward r spec, w spec (pivots recomputed on chip); backward r spec, INV
+        # (half a complex), w spec, and E if z is periodic
+        "k_spec_fwd": 2.0 * spec, "k_spec_bwd": (3.0 if not cfg["z_wall"] else 2.5) * spec,
         "k_fftx_inv": spec + 8.0, "k_correct": 56.0,
     }
     if heat:

@@ -343,19 +343,21 @@ extern "C" double fizzy_gamma(fizzy_ctx *c)
 namespace {
 
 // interface quantities of c->phi -> kappa, divRn (and Rn when rho1 != rho2): kernel group (a).
-// with_psi: psi and r = sqrt(q) of c->phi are not yet in c->psi / c->rr (fizzy_set_fields);
-// inside a substep k_phi_update has already written them.
+// with_psi: psi of c->phi is not yet in c->psi (fizzy_set_fields); inside a substep k_phi_update
+// has already written it.  r = sqrt(q) is recomputed on chip by the marching sweep; only the
+// tiny-grid fallback reads it from c->rr (k_iface_psi writes both).
 fizzy_status run_interface(fizzy_ctx *c, bool with_psi)
 {
     const FzP &P = c->P;
     dim3 grid, block;
     cell_launch(c, grid, block);
-    if (with_psi) {
+    const bool march = P.nx >= ITX && P.ny >= ITY;
+    if (with_psi || !march) {
         FZ_TB(FZK_IPSI);
         k_iface_psi<<<grid, block, 0, c->stream>>>(c->P, c->phi, c->psi, c->rr);
         FZ_LAUNCHED(FZK_IPSI);
     }
-    if (P.nx >= ITX && P.ny >= ITY) {   // marching sweep: nhat stays on chip
+    if (march) {   // marching sweep: nhat and r stay on chip
         int chunks = 8192 / ((P.nx / ITX) * (P.ny / ITY));
         if (chunks > P.nz / 16) chunks = P.nz / 16;
         if (chunks < 1) chunks = 1;
@@ -363,10 +365,10 @@ fizzy_status run_interface(fizzy_ctx *c, bool with_psi)
         const dim3 g(P.nx / ITX, P.ny / ITY, (P.nz + KC - 1) / KC);
         FZ_TB(FZK_IMARCH);
         if (c->varrho)
-            k_iface_march<true><<<g, dim3(ITX, ITY), IFACE_SMEM, c->stream>>>(P, c->psi, c->rr, c->phi, c->kappa, c->divrn,
+            k_iface_march<true><<<g, dim3(ITX, ITY), IFACE_SMEM, c->stream>>>(P, c->psi, c->phi, c->kappa, c->divrn,
                                                                               c->rnx, c->rny, c->rnz, KC);
         else
-            k_iface_march<false><<<g, dim3(ITX, ITY), IFACE_SMEM, c->stream>>>(P, c->psi, c->rr, c->phi, c->kappa, c->divrn,
+            k_iface_march<false><<<g, dim3(ITX, ITY), IFACE_SMEM, c->stream>>>(P, c->psi, c->phi, c->kappa, c->divrn,
                                                                                nullptr, nullptr, nullptr, KC);
         FZ_LAUNCHED(FZK_IMARCH);
         return FIZZY_OK;
@@ -500,8 +502,7 @@ extern "C" fizzy_status fizzy_rk3_substep(fizzy_ctx *c, int stage, double dt)
     }
     // S1: phi transport (divRn holds D(R/Gamma) of the current phi)
     FZ_TB(FZK_PHI);
-    k_phi_update<<<grid, block, 0, c->stream>>>(P, c->phi, c->u, c->v, c->w, c->divrn, c->hphi, c->phin, c->psi, c->rr, c->scal,
-                                                dt, gs, zs);
+    k_phi_update<<<grid, block, 0, c->stream>>>(P, c->phi, c->u, c->v, c->w, c->divrn, c->hphi, c->phin, c->psi, c->scal, dt, gs, zs, stage != 2);
     FZ_LAUNCHED(FZK_PHI);
     std::swap(c->phi, c->phin);
     // interface quantities of phi_new (N6): used by S3 now and by S1 of the next substep
@@ -509,7 +510,7 @@ extern "C" fizzy_status fizzy_rk3_substep(fizzy_ctx *c, int stage, double dt)
     // S2b: temperature
     if (c->heat) {
         FZ_TB(FZK_TEMP);
-        k_temp_update<<<grid, block, 0, c->stream>>>(P, c->T, c->phi, c->u, c->v, c->w, c->hT, c->Tn, dt, gs, zs);
+        k_temp_update<<<grid, block, 0, c->stream>>>(P, c->T, c->phi, c->u, c->v, c->w, c->hT, c->Tn, dt, gs, zs, stage != 2);
         FZ_LAUNCHED(FZK_TEMP);
         std::swap(c->T, c->Tn);
     }
@@ -518,7 +519,7 @@ extern "C" fizzy_status fizzy_rk3_substep(fizzy_ctx *c, int stage, double dt)
     A.u = c->u; A.v = c->v; A.w = c->w; A.phi = c->phi; A.kappa = c->kappa;
     A.rnx = c->rnx; A.rny = c->rny; A.rnz = c->rnz; A.p = c->p; A.pp = c->pp; A.T = c->T;
     A.us = c->us; A.vs = c->vs; A.ws = c->ws; A.hu = c->hu; A.hv = c->hv; A.hw = c->hw;
-    A.scal = c->scal; A.dt = dt; A.gs = gs; A.zs = zs; A.adt = as * dt;
+    A.scal = c->scal; A.dt = dt; A.gs = gs; A.zs = zs; A.adt = as * dt; A.keep_h = stage != 2;
     FZ_TB(FZK_MOM);
     if (c->varrho) { if (c->varmu) launch_momentum<true, true>(c, grid, block, A); else launch_momentum<true, false>(c, grid, block, A); }
     else { if (c->varmu) launch_momentum<false, true>(c, grid, block, A); else launch_momentum<false, false>(c, grid, block, A); }

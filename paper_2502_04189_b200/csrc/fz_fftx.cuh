@@ -24,8 +24,13 @@ __host__ __device__ constexpr int fx_pairs(int log2n, bool inverse)
 }
 __host__ __device__ constexpr int fx_minb(int log2n, bool inverse) { return (!inverse && log2n == 9) ? 5 : 3; }
 #define FX_LINE(n_) ((n_) + ((n_) >> 3))
+// shared memory of one line pair: two padded lines + 2 elements of skew, so that the buffers of consecutive
+// pairs start 8 banks apart and the (un)tangling accesses, which touch the same l in every pair, do not collide
+#define FX_PAIR(n_) (2 * FX_LINE(n_) + 2)
+// L2 prefetch distance in CTAs: the CTAs that launch about one residency later (3-5 CTAs on each of 148 SMs)
+#define FX_AHEAD 592
 
-__host__ __device__ inline size_t fz_fftx_smem(int log2n, bool inverse) { return (size_t)2 * fx_pairs(log2n, inverse) * FX_LINE(1 << log2n) * 16; }
+__host__ __device__ inline size_t fz_fftx_smem(int log2n, bool inverse) { return (size_t)fx_pairs(log2n, inverse) * FX_PAIR(1 << log2n) * 16; }
 
 template <bool DIV, int LOG2N>
 __global__ void __launch_bounds__(fx_pairs(LOG2N, false) * ((1 << LOG2N) / 8), fx_minb(LOG2N, false))
@@ -34,15 +39,25 @@ k_fftx_fwd(FzP P, const double *__restrict__ src, const double *__restrict__ us,
            double2 *__restrict__ spec, const double2 *__restrict__ tw)
 {
     extern __shared__ __align__(16) double2 smx[];
-    constexpr int n = 1 << LOG2N, T8 = n / 8, LN = FX_LINE(n), FX_PAIRS = fx_pairs(LOG2N, false);
+    constexpr int n = 1 << LOG2N, T8 = n / 8, LN = FX_LINE(n), PS = FX_PAIR(n), FX_PAIRS = fx_pairs(LOG2N, false);
     const int jt = threadIdx.x, g = threadIdx.y;
-    double2 *A = smx + (2 * g) * LN, *B = A + LN;
+    double2 *A = smx + g * PS, *B = A + LN;
     FzLineFFT<LOG2N, -1, false> fft;
     fft.init(tw, jt);
     const long long L0 = (long long)blockIdx.x * (2 * FX_PAIRS);   // first line of the CTA; 2*FX_PAIRS | ny
     const int k = (int)(L0 / P.ny), j0 = (int)(L0 - (long long)k * P.ny);
     const int ja = j0 + 2 * g;                                      // lines ja (real part), ja+1 (imaginary part)
     const long long ra = ((long long)k * P.ny + ja) * n, rb = ra + n;
+    {   // pull the input lines of the CTA FX_AHEAD launches later into L2 (one 128-byte line per thread and array):
+        // this CTA's own loads were prefetched the same way, so the load phase sees L2, not HBM, latency
+        const long long Lp = L0 + (long long)FX_AHEAD * (2 * FX_PAIRS);
+        const int tq = g * T8 + jt;                                 // 16 doubles per 128-byte line
+        if (Lp < (long long)P.ny * P.nz && tq * 16 < 2 * FX_PAIRS * n) {
+            const long long o = Lp * n + tq * 16;
+            if (DIV) { fz_prefetch_l2(us + o); fz_prefetch_l2(vs + o); fz_prefetch_l2(ws + o); }
+            else fz_prefetch_l2(src + o);
+        }
+    }
     double2 v[8];
     if (DIV) {
         const long long rm = ((long long)k * P.ny + fz_im(ja, P.ny)) * n;   // row ja-1 (periodic)
@@ -69,7 +84,7 @@ k_fftx_fwd(FzP P, const double *__restrict__ src, const double *__restrict__ us,
     double2 *out = spec + (long long)k * nxh * P.ny + j0;
     for (int e = t; e < 2 * FX_PAIRS * nxh; e += nth) {
         const int l = e / (2 * FX_PAIRS), ln = e - l * (2 * FX_PAIRS);
-        const double2 *buf = smx + (2 * (ln >> 1)) * LN + roff;
+        const double2 *buf = smx + (ln >> 1) * PS + roff;
         const double2 z1 = buf[FZL_PADI(l)];
         const int l2 = (n - l) & (n - 1);
         const double2 z2 = buf[FZL_PADI(l2)];
@@ -89,9 +104,9 @@ k_fftx_inv(FzP P, const double2 *__restrict__ spec, double *__restrict__ dst, do
            const double2 *__restrict__ tw, const double *__restrict__ scal)
 {
     extern __shared__ __align__(16) double2 smx[];
-    constexpr int n = 1 << LOG2N, T8 = n / 8, LN = FX_LINE(n), FX_PAIRS = fx_pairs(LOG2N, true);
+    constexpr int n = 1 << LOG2N, T8 = n / 8, LN = FX_LINE(n), PS = FX_PAIR(n), FX_PAIRS = fx_pairs(LOG2N, true);
     const int jt = threadIdx.x, g = threadIdx.y;
-    double2 *A = smx + (2 * g) * LN, *B = A + LN;
+    double2 *A = smx + g * PS, *B = A + LN;
     FzLineFFT<LOG2N, +1, false> fft;
     fft.init(tw, jt);
     const long long L0 = (long long)blockIdx.x * (2 * FX_PAIRS);
@@ -100,11 +115,19 @@ k_fftx_inv(FzP P, const double2 *__restrict__ spec, double *__restrict__ dst, do
     const int nth = T8 * FX_PAIRS, t = g * T8 + jt;
     const int nxh = P.nxh;
     const double2 *in = spec + (long long)k * nxh * P.ny + j0;
+    {   // L2 prefetch of the spectrum rows of the CTA FX_AHEAD launches later (2*FX_PAIRS*16 bytes per l)
+        const long long Lp = L0 + (long long)FX_AHEAD * (2 * FX_PAIRS);
+        if (Lp < (long long)P.ny * P.nz) {
+            const int kp = (int)(Lp / P.ny), jp = (int)(Lp - (long long)kp * P.ny);
+            const double2 *inp = spec + (long long)kp * nxh * P.ny + jp;
+            for (int l = t; l < nxh; l += nth) fz_prefetch_l2(inp + (long long)l * P.ny);
+        }
+    }
     // tangle: consecutive threads -> consecutive pairs (32-byte pieces, runs of 2*FX_PAIRS*16 bytes per l)
     for (int e = t; e < FX_PAIRS * nxh; e += nth) {
         const int l = e / FX_PAIRS, pr = e - l * FX_PAIRS;
         const double2 a = in[(long long)l * P.ny + 2 * pr], b = in[(long long)l * P.ny + 2 * pr + 1];
-        double2 *buf = smx + (2 * pr) * LN;
+        double2 *buf = smx + pr * PS;
         if (l == 0 || l == n / 2) {
             buf[FZL_PADI(l)] = make_double2(a.x, b.x);
         } else {

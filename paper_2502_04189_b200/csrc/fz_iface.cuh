@@ -1,21 +1,24 @@
 // fz_iface.cuh -- kernel group (a): interface quantities of a phase field in ONE marching sweep.
-// Inputs psi = eps ln q, r = sqrt q (written pointwise by the kernel that produced phi) and phi;
-// outputs kappa = -D(nf), divRn = D(R/Gamma) and, when rho1 != rho2, Rn on the three "+" faces
-// (BASELINE.json:5(i),(iii); readings N3-N5).  The cell-centred normal nhat = G/max(|G|,1e-30)
-// is computed ONCE per cell on chip and shared through shared memory -- it never goes to HBM.
+// Inputs psi = eps ln q (written pointwise by the kernel that produced phi) and phi; outputs
+// kappa = -D(nf), divRn = D(R/Gamma) and, when rho1 != rho2, Rn on the three "+" faces
+// (BASELINE.json:5(i),(iii); readings N3-N5).  The cell-centred normal nhat = G/max(|G|,1e-30) and
+// r = sqrt(q) are computed ONCE per cell on chip and shared through shared memory -- they never go
+// to HBM (r is a pointwise function of phi: one reciprocal and one rsqrt per staged cell).
 //
 // A CTA owns an x-y tile of ITX x ITY cells and marches over a chunk of z planes.  Shared memory
-// holds rings of four planes of psi, r, phi (tile + halo 2) and of the HALF normals 0.5 nhat_x,
-// 0.5 nhat_y (tile + halo 1); nhat_z of the thread's own column and the z face below it live in
-// registers.  Planes arrive by 16-byte cp.async (LDGSTS), so no register is tied up by a load in
-// flight.  Step kk: (1) wait for plane kk+1, (2) barrier, (3) issue the copies of plane kk+2,
-// (4) half normals of plane kk for the tile and its halo-1 cross, (5) plane kk-1 is finished and
-// written.  One barrier per plane.  The plane loop is unrolled by four so that every ring slot is a
-// COMPILE-TIME constant: all shared-memory accesses are [thread base + immediate] and the ring /
-// address arithmetic of a rolled loop (a third of its instructions) disappears.
-// Slot of plane p = (p - (k0 - 2)) & 3, step s = kk - (k0 - 1):
-//   psi, r, phi:  planes kk-1, kk, kk+1 in slots s, s+1, s+2 (mod 4); plane kk+2 is issued into slot s+3
-//   half normals: plane kk is written into slot s+1, plane k = kk-1 is read from slot s.
+// holds rings of IRING planes of psi and phi (tile + halo 2), of three planes of r (tile + halo 1)
+// and of two planes of the HALF normals 0.5 nhat_x, 0.5 nhat_y (tile + halo 1); nhat_z of the
+// thread's own column and the z face below it live in registers.  Planes arrive by 16-byte cp.async
+// (LDGSTS) issued IDEPTH = IRING-3 planes ahead of their first use, so no register is tied up by a
+// load in flight and HBM latency under load (several microseconds) hides behind IDEPTH planes of
+// compute.  Step s (kk = k0-2+s): (1) wait for plane kk+1, (2) barrier, (3) issue the copies of
+// plane kk+1+IDEPTH into the slot plane kk-2 just left, (4) r of plane kk+1, (5) half normals of
+// plane kk for the tile and its halo-1 cross, (6) plane k = kk-1 is finished and written.  One
+// barrier per plane.  The plane loop is unrolled by IRING (a multiple of 2 and 3) so that every ring
+// slot is a COMPILE-TIME constant: all shared-memory accesses are [thread base + immediate].
+//   psi, phi:     planes kk-1, kk, kk+1 in slots (s-1, s, s+1) mod IRING
+//   r:            plane kk+1 is written into slot (s+1) mod 3; planes kk-1, kk are read from (s-1, s) mod 3
+//   half normals: plane kk is written into slot s mod 2, plane k = kk-1 is read from slot (s-1) mod 2
 #pragma once
 #include <type_traits>
 #include "fz_common.cuh"
@@ -28,9 +31,13 @@
 #define INW (ITX + 2)
 #define INH (ITY + 2)
 #define INS (INW * INH)
-#define I4RING 4
+#ifndef IRING
+#define IRING 6
+#endif
+#define IDEPTH (IRING - 3)
 #define ICHUNKS (IPS / 2)   // 16-byte chunks of one staged plane
-#define IFACE_SMEM ((3 * I4RING * IPS + 2 * I4RING * INS) * sizeof(double))
+#define IFACE_SMEM ((2 * IRING * IPS + 7 * INS) * sizeof(double))   // psi, phi rings + 3 planes of r + 2 x (nhx, nhy)
+static_assert(IRING % 6 == 0, "the plane loop is unrolled by IRING: ring slots of depth 2 and 3 must be compile-time too");
 
 // 1/(1+s)^2 * s with one reciprocal: sharpening coefficient 1/4 (1 - tanh^2((psi_a+psi_b)/(4 eps)))
 // = s/(1+s)^2, s = r_a r_b (D1)
@@ -41,20 +48,30 @@ __device__ __forceinline__ double fz_sharp2(double ra, double rb)
     return s * t * t;
 }
 
+// r = sqrt(q), q = (phic + delta)/(1 - phic + delta) (N2); 1 - phic + delta in [delta, 1 + delta], q in
+// [delta, 1/delta] with delta >= 1e-150 (fizzy_create): all normal, so the branch-free helpers apply
+__device__ __forceinline__ double fz_sqrtq(double phi, double delta)
+{
+    const double ph = fz_clip01(phi);
+    const double q = (ph + delta) * fz_rcp(1.0 - ph + delta);
+    return q * fz_rsqrt(q);
+}
+
 template <bool STORE_R>
 __global__ void __launch_bounds__(ITX * ITY, 2)
-k_iface_march(FzP P, const double *__restrict__ psi, const double *__restrict__ rr,
-               const double *__restrict__ phi, double *__restrict__ kappa, double *__restrict__ divrn,
+k_iface_march(FzP P, const double *__restrict__ psi, const double *__restrict__ phi,
+               double *__restrict__ kappa, double *__restrict__ divrn,
                double *__restrict__ rnx, double *__restrict__ rny, double *__restrict__ rnz, int KC)
 {
     extern __shared__ __align__(16) double smi[];
     const int tx = threadIdx.x, ty = threadIdx.y, t = ty * ITX + tx;
     const int i0 = blockIdx.x * ITX, j0 = blockIdx.y * ITY;
     const int k0 = blockIdx.z * KC, k1 = min(k0 + KC, P.nz);
-    // per-thread base pointers: own cell in a psi / r / phi plane, own cell in a half-normal plane
+    // per-thread base pointers: own cell in a psi / phi plane, own cell in an r / half-normal plane
     const double *PSIc = smi + (ty + 2) * IPW + tx + 2;
-    const double *RRc = PSIc + I4RING * IPS, *PHIc = RRc + I4RING * IPS;
-    double *NHXc = smi + 3 * I4RING * IPS + (ty + 1) * INW + tx + 1, *NHYc = NHXc + I4RING * INS;
+    const double *PHIc = PSIc + IRING * IPS;
+    double *RRc = smi + 2 * IRING * IPS + (ty + 1) * INW + tx + 1;
+    double *NHXc = RRc + 3 * INS, *NHYc = NHXc + INS;   // [slot 0: x, y][slot 1: x, y]
     // staging map (16-byte chunks of the tile + halo 2 rectangle)
     const bool loader = t < ICHUNKS;
     const int lrow = t / (IPW / 2), lcp = t - lrow * (IPW / 2);
@@ -62,28 +79,29 @@ k_iface_march(FzP P, const double *__restrict__ psi, const double *__restrict__ 
     double *stg = smi + lrow * IPW + 2 * lcp;
     const int zlo = P.z_wall ? -1 : P.nz, zhi = P.z_wall ? 2 * P.nz - 1 : -P.nz, zsg = P.z_wall ? -1 : 1;
     const unsigned sxy = (unsigned)P.sxy;
-    // plane kk of psi, r, phi -> ring slot `slot` (compile-time in the loop)
+    // plane kk of psi, phi -> ring slot `slot` (compile-time in the loop)
     auto issue = [&](int kk, int slot) {
         if (loader) {
             const int zs = kk < 0 ? zlo + zsg * kk : (kk >= P.nz ? zhi + zsg * kk : kk);
             const unsigned g = (unsigned)zs * sxy + ugoff;
             double *d = stg + slot * IPS;
             fz_cp_async16(d, psi + g);
-            fz_cp_async16(d + I4RING * IPS, rr + g);
-            fz_cp_async16(d + 2 * I4RING * IPS, phi + g);
+            fz_cp_async16(d + IRING * IPS, phi + g);
         }
     };
-    // halo-1 cross cell of the half-normal plane handled by this thread (threads 0 .. 95)
+    // halo-1 cross cell of the r / half-normal planes handled by this thread (threads 0 .. 95)
     int hr = 1, hc = 2;
     const bool has_h = t < 2 * (ITX + ITY);
     if (t < ITX) { hr = 1; hc = 2 + t; }
     else if (t < 2 * ITX) { hr = ITY + 2; hc = 2 + t - ITX; }
     else if (t < 2 * ITX + ITY) { hr = 2 + t - 2 * ITX; hc = 1; }
     else if (has_h) { hr = 2 + t - 2 * ITX - ITY; hc = ITX + 2; }
-    const double *PSIh = smi + hr * IPW + hc;
-    double *NHXh = smi + 3 * I4RING * IPS + (hr - 1) * INW + hc - 1, *NHYh = NHXh + I4RING * INS;
+    const double *PSIh = smi + hr * IPW + hc, *PHIh = PSIh + IRING * IPS;
+    double *RRh = smi + 2 * IRING * IPS + (hr - 1) * INW + hc - 1;
+    double *NHXh = RRh + 3 * INS, *NHYh = NHXh + INS;
     const double hx = 0.5 * P.idx, hy = 0.5 * P.idy;
     const double ex = P.eps * P.idx, ey = P.eps * P.idy;
+    const double delta = P.delta;
     // HALF normal 0.5 G / max(|G|, 1e-30) (N4) of the cell at q, psi planes at slots SM, S0, SP
     auto normal = [&](const double *q, int om, int o0, int op, double igz, double &nx_, double &ny_, double &nz_) {
         const double gx = (q[o0 + 1] - q[o0 - 1]) * hx;
@@ -93,22 +111,32 @@ k_iface_march(FzP P, const double *__restrict__ psi, const double *__restrict__ 
         nx_ = gx * inv; ny_ = gy * inv; nz_ = gz * inv;
     };
 
-    issue(k0 - 2, 0); issue(k0 - 1, 1); issue(k0, 2);
+    // prologue: planes k0-2 .. k0-2+IDEPTH in IDEPTH groups (the first holds two planes)
+    issue(k0 - 2, 0); issue(k0 - 1, 1);
     fz_cp_async_commit();
+#pragma unroll
+    for (int d = 2; d <= IDEPTH; ++d) { issue(k0 - 2 + d, d); fz_cp_async_commit(); }
     double nz0 = 0.0, nzp = 0.0, nfz_prev = 0.0, Rz_prev = 0.0;
     const unsigned gc = (unsigned)((i0 + tx) + P.nx * (j0 + ty));
-    double igz_n = P.igz[k0 - 1], idzc_n = P.idzc[k0 - 2], idzf_n = P.idzf[k0 - 2];   // z metrics: one step ahead
+    double igz_n = P.igz[k0 - 2], idzc_n = 0.0, idzf_n = 0.0;   // z metrics: loaded one step ahead (plane k0-3 is never used)
     auto step = [&](auto Sc, int kk) {
         constexpr int S = decltype(Sc)::value;
-        constexpr int om = S * IPS, o0 = ((S + 1) & 3) * IPS, op = ((S + 2) & 3) * IPS;   // psi/r/phi planes kk-1, kk, kk+1
-        constexpr int nm = S * INS, n0 = ((S + 1) & 3) * INS;                              // half-normal planes kk-1, kk
-        fz_cp_async_wait<0>();
+        constexpr int om = ((S + IRING - 1) % IRING) * IPS, o0 = (S % IRING) * IPS, op = ((S + 1) % IRING) * IPS;
+        constexpr int rm = ((S + 2) % 3) * INS, r0s = (S % 3) * INS, rp = ((S + 1) % 3) * INS;   // r planes kk-1, kk, kk+1
+        constexpr int n0 = (S % 2) * 2 * INS, nm = ((S + 1) % 2) * 2 * INS;                       // half-normal planes kk, kk-1
+        fz_cp_async_wait<IDEPTH - 1>();
         __syncthreads();
-        if (kk + 2 <= k1 + 1) issue(kk + 2, (S + 3) & 3);
+        if (kk + 1 + IDEPTH <= k1 + 1) issue(kk + 1 + IDEPTH, (S + IRING - 2) % IRING);
         fz_cp_async_commit();
+        // r = sqrt(q) of plane kk+1: own cell and the halo cross
+        RRc[rp] = fz_sqrtq(PHIc[op], delta);
+        if (has_h) RRh[rp] = fz_sqrtq(PHIh[op], delta);
+        const double igz = igz_n;
+        igz_n = P.igz[kk + 1];
+        const double idzc_k = idzc_n, idzf_k = idzf_n;   // metrics of plane k = kk-1, loaded one step ago
+        idzc_n = P.idzc[kk]; idzf_n = P.idzf[kk];
+        if (kk < k0 - 1) return;
         {   // half normals of plane kk: own cell, then the halo cross
-            const double igz = igz_n;
-            igz_n = P.igz[kk + 1];
             double ax, ay, az;
             normal(PSIc, om, o0, op, igz, ax, ay, az);
             NHXc[n0] = ax; NHYc[n0] = ay;
@@ -119,30 +147,29 @@ k_iface_march(FzP P, const double *__restrict__ psi, const double *__restrict__ 
             }
         }
         const int k = kk - 1;
-        const double idzc_k = idzc_n, idzf_k = idzf_n;   // metrics of plane k, loaded one step ago
-        idzc_n = P.idzc[kk]; idzf_n = P.idzf[kk];
         if (k < k0 - 1) return;
-        const double f0 = PHIc[om], r0 = RRc[om];
+        const double f0 = PHIc[om], r0 = RRc[rm];
         // z face k+1/2: zero on a wall face; the face k-1/2 is carried in registers
         const double zf = (P.z_wall && (k == -1 || k == P.nz - 1)) ? 0.0 : 1.0;
         const double nfzp = zf * (nz0 + nzp);
-        const double Rzp = zf * (P.eps * (PHIc[o0] - f0) * idzc_k - fz_sharp2(r0, RRc[o0]) * nfzp);
+        const double Rzp = zf * (P.eps * (PHIc[o0] - f0) * idzc_k - fz_sharp2(r0, RRc[r0s]) * nfzp);
         if (k < k0) { nfz_prev = nfzp; Rz_prev = Rzp; return; }
         // half normals of plane k were written one step ago: visible after this step's barrier
         const double ax = NHXc[nm], ay = NHYc[nm];
         const double nfxp = ax + NHXc[nm + 1], nfxm = NHXc[nm - 1] + ax;
         const double nfyp = ay + NHYc[nm + INW], nfym = NHYc[nm - INW] + ay;
-        const double Rxp = ex * (PHIc[om + 1] - f0) - fz_sharp2(r0, RRc[om + 1]) * nfxp;
-        const double Rxm = ex * (f0 - PHIc[om - 1]) - fz_sharp2(RRc[om - 1], r0) * nfxm;
-        const double Ryp = ey * (PHIc[om + IPW] - f0) - fz_sharp2(r0, RRc[om + IPW]) * nfyp;
-        const double Rym = ey * (f0 - PHIc[om - IPW]) - fz_sharp2(RRc[om - IPW], r0) * nfym;
+        const double Rxp = ex * (PHIc[om + 1] - f0) - fz_sharp2(r0, RRc[rm + 1]) * nfxp;
+        const double Rxm = ex * (f0 - PHIc[om - 1]) - fz_sharp2(RRc[rm - 1], r0) * nfxm;
+        const double Ryp = ey * (PHIc[om + IPW] - f0) - fz_sharp2(r0, RRc[rm + INW]) * nfyp;
+        const double Rym = ey * (f0 - PHIc[om - IPW]) - fz_sharp2(RRc[rm - INW], r0) * nfym;
         const unsigned c = (unsigned)k * sxy + gc;
         kappa[c] = -((nfxp - nfxm) * P.idx + (nfyp - nfym) * P.idy + (nfzp - nfz_prev) * idzf_k);
         divrn[c] = (Rxp - Rxm) * P.idx + (Ryp - Rym) * P.idy + (Rzp - Rz_prev) * idzf_k;
         if (STORE_R) { rnx[c] = Rxp; rny[c] = Ryp; rnz[c] = Rzp; }
         nfz_prev = nfzp; Rz_prev = Rzp;
     };
-    for (int kk = k0 - 1; kk <= k1; kk += 4) {
+    // steps kk = k0-2 .. k1 (plane k = kk-1 = k1-1 is the last one written)
+    for (int kk = k0 - 2; kk <= k1; kk += IRING) {
         step(std::integral_constant<int, 0>{}, kk);
         if (kk + 1 > k1) break;
         step(std::integral_constant<int, 1>{}, kk + 1);
@@ -150,6 +177,10 @@ k_iface_march(FzP P, const double *__restrict__ psi, const double *__restrict__ 
         step(std::integral_constant<int, 2>{}, kk + 2);
         if (kk + 3 > k1) break;
         step(std::integral_constant<int, 3>{}, kk + 3);
+        if (kk + 4 > k1) break;
+        step(std::integral_constant<int, 4>{}, kk + 4);
+        if (kk + 5 > k1) break;
+        step(std::integral_constant<int, 5>{}, kk + 5);
     }
     fz_cp_async_wait<0>();
 }

@@ -15,6 +15,7 @@ struct FzMomArgs {
     double *us, *vs, *ws, *hu, *hv, *hw;
     const double *scal;  // scal[1] = Gamma
     double dt, gs, zs, adt;  // adt = (gs+zs)*dt
+    int keep_h;              // 0 at stage 2: the next stage has zeta = 0 and never reads the history
 };
 
 template <bool VARRHO, bool VARMU, bool HEAT>
@@ -117,7 +118,7 @@ k_momentum(FzP P, FzMomArgs A)
         double un = u000 + A.dt * (A.gs * rhs + A.zs * A.hu[c]);
         if (VARRHO) un -= A.adt * (irx - ir0) * (php00 - ph000) * dx;
         A.us[c] = un;
-        A.hu[c] = rhs;
+        if (A.keep_h) A.hu[c] = rhs;
     }
     // ================= y component, face (i, j+1/2, k) =================
     {
@@ -147,7 +148,7 @@ k_momentum(FzP P, FzMomArgs A)
         double vn = v000 + A.dt * (A.gs * rhs + A.zs * A.hv[c]);
         if (VARRHO) vn -= A.adt * (iry - ir0) * (ph0p0 - ph000) * dy;
         A.vs[c] = vn;
-        A.hv[c] = rhs;
+        if (A.keep_h) A.hv[c] = rhs;
     }
     // ================= z component, face (i, j, k+1/2) =================
     if (k < P.kzf) {
@@ -180,10 +181,10 @@ k_momentum(FzP P, FzMomArgs A)
         double wn = w000 + A.dt * (A.gs * rhs + A.zs * A.hw[c]);
         if (VARRHO) wn -= A.adt * (irz - ir0) * (ph00p - ph000) * izc;
         A.ws[c] = wn;
-        A.hw[c] = rhs;
+        if (A.keep_h) A.hw[c] = rhs;
     } else {
         A.ws[c] = 0.0;
-        A.hw[c] = 0.0;
+        if (A.keep_h) A.hw[c] = 0.0;
     }
 }
 
@@ -372,7 +373,7 @@ k_momentum_march(FzP P, FzMomArgs A, int KC)
             double un = u000 + A.dt * (A.gs * rhs + A.zs * hu_old);
             if (VARRHO) un -= A.adt * (irx - ir0) * (php00 - ph000) * dx;
             A.us[c] = un;
-            A.hu[c] = rhs;
+            if (A.keep_h) A.hu[c] = rhs;
         }
         // ================= y component =================
         {
@@ -400,7 +401,7 @@ k_momentum_march(FzP P, FzMomArgs A, int KC)
             double vn = v000 + A.dt * (A.gs * rhs + A.zs * hv_old);
             if (VARRHO) vn -= A.adt * (iry - ir0) * (ph0p0 - ph000) * dy;
             A.vs[c] = vn;
-            A.hv[c] = rhs;
+            if (A.keep_h) A.hv[c] = rhs;
         }
         // ================= z component =================
         if (k < P.kzf) {
@@ -431,10 +432,10 @@ k_momentum_march(FzP P, FzMomArgs A, int KC)
             double wn = w000 + A.dt * (A.gs * rhs + A.zs * hw_old);
             if (VARRHO) wn -= A.adt * (irz - ir0) * (ph00p - ph000) * izc;
             A.ws[c] = wn;
-            A.hw[c] = rhs;
+            if (A.keep_h) A.hw[c] = rhs;
         } else {
             A.ws[c] = 0.0;
-            A.hw[c] = 0.0;
+            if (A.keep_h) A.hw[c] = 0.0;
         }
 #undef S_
 #undef MUE_

@@ -41,6 +41,12 @@ struct FzTri {
 #define SPEC_PADI(i_) ((i_) + ((i_) >> 3))
 #define SPEC_LINE(n_) ((n_) + ((n_) >> 3))
 
+// pivot of row k: b_k + lam - a_k c'_{k-1}, b_k = -(a_k + c_k); one spelling for the table and the kernels
+__device__ __forceinline__ double fz_tri_den(double a, double c, double lam, double cp)
+{
+    return fma(-a, cp, lam - (a + c));
+}
+
 __global__ void k_tri_tables(FzP P, FzTri Tt)
 {
     const long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x;
@@ -53,8 +59,8 @@ __global__ void k_tri_tables(FzP P, FzTri Tt)
         double cp = 0.0;
         for (int k = 0; k < n; ++k) {
             const double a = Tt.a[k], c = Tt.c[k];
-            const double den = -(a + c) + lam - a * cp;
-            double inv = 1.0 / den;
+            const double den = fz_tri_den(a, c, lam, cp);
+            double inv = fz_rcp_signed(den);      // the same pivot, bit for bit, that k_spec_fwd recomputes
             if (t == 0 && k == n - 1) inv = 0.0;  // N17: x_{nz-1} = 0 for the singular mode
             Tt.inv[(long long)k * M + t] = inv;
             cp = c * inv;
@@ -66,8 +72,8 @@ __global__ void k_tri_tables(FzP P, FzTri Tt)
         for (int k = 0; k <= n - 2; ++k) {
             const double a = Tt.a[k];
             const double c = (k == n - 2) ? 0.0 : Tt.c[k];
-            const double den = -(Tt.a[k] + Tt.c[k]) + lam - a * cp;
-            const double inv = 1.0 / den;
+            const double den = fz_tri_den(a, Tt.c[k], lam, cp);
+            const double inv = fz_rcp_signed(den);
             double ek = (k == 0) ? a * inv : -a * e * inv;
             if (k == n - 2) ek += Tt.c[k] * inv;   // c_{n-2} multiplies X as well
             const double fk = (k == n - 2) ? f + Tt.a[n - 1] : f;
@@ -84,10 +90,11 @@ __global__ void k_tri_tables(FzP P, FzTri Tt)
     }
 }
 
-// shared memory: scratch line | ring of SPEC_RING padded lines | ring of INV rows (| ring of E rows)
-__host__ __device__ inline size_t fz_spec_smem(int n, bool with_e)
+// shared memory: scratch line | ring of SPEC_RING padded lines | `tables` rings of coefficient rows
+// (forward sweep: none; backward: INV, and E when z is periodic)
+__host__ __device__ inline size_t fz_spec_smem(int n, int tables)
 {
-    return (size_t)SPEC_LINE(n) * 16 + (size_t)SPEC_RING * ((size_t)SPEC_LINE(n) * 16 + (size_t)n * 8 * (with_e ? 2 : 1));
+    return (size_t)SPEC_LINE(n) * 16 + (size_t)SPEC_RING * ((size_t)SPEC_LINE(n) * 16 + (size_t)n * 8 * tables);
 }
 
 // ---------------------------------------------------------------- forward: FFT_y + elimination
@@ -100,7 +107,6 @@ k_spec_fwd(FzP P, FzTri Tt, double2 *__restrict__ spec, const double2 *__restric
     constexpr int n = 1 << LOG2N, nt = n / 8, LN = SPEC_LINE(n);
     const int jt = threadIdx.x, nz = P.nz;
     double2 *scratch = sms, *lines = sms + LN;
-    double *invs = reinterpret_cast<double *>(lines + SPEC_RING * LN);
     FzLineFFT<LOG2N, -1> fft;
     fft.init(tw, jt);
     const long long M = (long long)P.nxh * n, base = (long long)blockIdx.x * n;
@@ -111,34 +117,37 @@ k_spec_fwd(FzP P, FzTri Tt, double2 *__restrict__ spec, const double2 *__restric
             double2 *d = lines + slot * LN;
 #pragma unroll
             for (int q = 0; q < 8; ++q) { const int i = jt + q * nt; fz_cp_async16(d + SPEC_PADI(i), g + i); }
-            const double *gi = Tt.inv + (long long)k * M + base;
-            double *di = invs + slot * n;
-#pragma unroll
-            for (int q = 0; q < 4; ++q) { const int i = 2 * (jt + q * nt); fz_cp_async16(di + i, gi + i); }
         }
     };
     for (int p = 0; p < SPEC_RING - 1; ++p) { issue(p); fz_cp_async_commit(); }
     double2 dp[8], h[8], v[8];
-    double f[8];
+    double f[8], lam[8], cp[8];   // the pivots are recomputed on the fly (c' carried): the forward sweep reads no table
     const double c_last = Tt.c[nz - 1], a_last = Tt.a[nz - 1];
+    const double lamx = Tt.lamx[blockIdx.x];
 #pragma unroll
-    for (int q = 0; q < 8; ++q) { dp[q] = make_double2(0, 0); h[q] = make_double2(0, 0); f[q] = c_last; }
+    for (int q = 0; q < 8; ++q) {
+        dp[q] = make_double2(0, 0); h[q] = make_double2(0, 0); f[q] = c_last;
+        lam[q] = lamx + Tt.lamy[jt + q * nt]; cp[q] = 0.0;
+    }
     for (int k = 0; k < nz; ++k) {
         fz_cp_async_wait<SPEC_RING - 2>();
         __syncthreads();
         issue(k + SPEC_RING - 1);
         fz_cp_async_commit();
         fft.smem_to_regs(jt, lines + (k & (SPEC_RING - 1)) * LN, scratch, v);
-        const double *iv = invs + (k & (SPEC_RING - 1)) * n;
         double2 *out = spec + (long long)k * M + base;
-        const double a = Tt.a[k];
+        const double a = Tt.a[k], cfull = Tt.c[k];
         if (!CYCLIC || k < nz - 1) {
             const bool pen = CYCLIC && k == nz - 2;       // row nz-2 of a cyclic system
-            const double ck = pen ? 0.0 : Tt.c[k], fadd = pen ? a_last : 0.0;
+            const double ck = pen ? 0.0 : cfull, fadd = pen ? a_last : 0.0;
+            // N17: x_{nz-1} = 0 for the singular mode (walls); its thread is (l, m) = (0, 0), q = 0
+            const bool sing = !CYCLIC && k == nz - 1 && blockIdx.x == 0 && jt == 0;
 #pragma unroll
             for (int q = 0; q < 8; ++q) {
                 const int m = jt + q * nt;
-                const double inv = iv[m];
+                double inv = fz_rcp_signed(fz_tri_den(a, cfull, lam[q], cp[q]));
+                if (q == 0 && sing) inv = 0.0;
+                cp[q] = ck * inv;
                 dp[q].x = (v[q].x - a * dp[q].x) * inv;
                 dp[q].y = (v[q].y - a * dp[q].y) * inv;
                 if (CYCLIC) {
@@ -243,7 +252,7 @@ cudaError_t fz_spec_launch_one(bool fwd, const FzP &P, const FzTri &Tt, double2 
                                double *scal, cudaStream_t st)
 {
     const int n = 1 << LOG2N;
-    const size_t smem = fz_spec_smem(n, fwd ? false : CYCLIC);
+    const size_t smem = fz_spec_smem(n, fwd ? 0 : (CYCLIC ? 2 : 1));
     cudaError_t e;
     if (fwd) {
         e = cudaFuncSetAttribute(k_spec_fwd<CYCLIC, LOG2N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);

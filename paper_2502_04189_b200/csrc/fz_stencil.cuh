@@ -115,13 +115,12 @@ __global__ void k_iface_flux(FzP P, const double *__restrict__ phi, const double
 
 // ---------------------------------------------------------------- S1: ACDI phi transport
 // RHSphi = D(-u_a phibar_a) + Gamma D(Rn);  phi <- phi + dt (g RHS + z RHS_old)   (BASELINE.json:5(i))
-// also writes psi = eps ln q and r = sqrt q of phi_new (N2), the inputs of k_iface_march
+// also writes psi = eps ln q of phi_new (N2), the input of k_iface_march (r = sqrt q is recomputed there)
 __global__ void k_phi_update(FzP P, const double *__restrict__ phi, const double *__restrict__ u,
                              const double *__restrict__ v, const double *__restrict__ w,
                              const double *__restrict__ divrn, double *__restrict__ hphi,
                              double *__restrict__ phin, double *__restrict__ psi,
-                             double *__restrict__ rr, const double *__restrict__ scal, double dt,
-                             double gs, double zs)
+                             const double *__restrict__ scal, double dt, double gs, double zs, int keep_h)
 {
     FZ_CELL_IJK
     const FzZ z = fz_zn(P, k);
@@ -139,12 +138,11 @@ __global__ void k_phi_update(FzP P, const double *__restrict__ phi, const double
     // stage 0 has zeta = 0: the history is not read (it may hold anything finite; 0 * h == 0)
     const double fn = f0 + dt * (gs * rhs + (zs != 0.0 ? zs * hphi[c] : 0.0));
     phin[c] = fn;
-    hphi[c] = rhs;
-    // psi, r = sqrt(q) of phi_new for the interface sweep (same formulas as k_iface_psi)
+    if (keep_h) hphi[c] = rhs;   // not at stage 2: the next stage has zeta = 0 and never reads it
+    // psi of phi_new for the interface sweep (same formula as k_iface_psi)
     const double ph = fz_clip01(fn);
     const double q = (ph + P.delta) / (1.0 - ph + P.delta);
     psi[c] = P.eps * log(q);
-    rr[c] = sqrt(q);
 }
 
 // ---------------------------------------------------------------- S2b: temperature transport (N14)
@@ -154,7 +152,7 @@ __global__ void __launch_bounds__(256, 6)
 k_temp_update(FzP P, const double *__restrict__ T, const double *__restrict__ phi,
               const double *__restrict__ u, const double *__restrict__ v,
               const double *__restrict__ w, double *__restrict__ hT,
-              double *__restrict__ Tn, double dt, double gs, double zs)
+              double *__restrict__ Tn, double dt, double gs, double zs, int keep_h)
 {
     FZ_CELL_IJK
     const FzZ z = fz_zn(P, k);
@@ -189,7 +187,7 @@ k_temp_update(FzP P, const double *__restrict__ T, const double *__restrict__ ph
     const double rcp = (P.rho2 + P.drho * phc) * (P.cp2 + (P.cp1 - P.cp2) * phc);
     const double rhs = adv + dif * fz_rcp(rcp);
     Tn[c] = t0 + dt * (gs * rhs + (zs != 0.0 ? zs * hT[c] : 0.0));
-    hT[c] = rhs;
+    if (keep_h) hT[c] = rhs;
 }
 
 // ---------------------------------------------------------------- S5: velocity correction

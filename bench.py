@@ -10,7 +10,13 @@ target is quoted on), synthetic seeded inputs from paper_2502_04189_b200.workloa
 N>1: replicas only: every rank runs the same workload on its own GPU,
 no data-path collective; value = cells*substeps of all ranks / max-over-ranks time.
 
-One JSON line on stdout (rank 0).  `--impl reference` times the CPU oracle on a bounded sample.
+One JSON line on stdout (rank 0).  `--impl reference` times the CPU oracle on a bounded sample
+(the same recipe at --cpu-grid^3, the grid the `cpu_baseline` leg of the default arm uses too).
+
+Timed regions: (1) `value`: K steps, inputs resident in HBM, per-kernel timing OFF, CUDA events on the
+library's stream; (2) a second, shorter pass with fizzy_timing_enable for the per-kernel table and the
+`roofline` object; (3) `e2e`: host buffers through the C ABI; (4) `cufft_compare`: cuFFT (torch.fft)
+on the transforms of S4 only, bench-only yardstick -- cuFFT is never used by libfizzy.so.
 """
 from __future__ import annotations
 
@@ -29,6 +35,7 @@ sys.path.insert(0, ROOT)
 
 from paper_2502_04189_b200 import workloads as W  # noqa: E402
 
+TRAFFIC_CSV, TRAFFIC_MD = "r2_traffic.csv", "r2_ncu_full.md"
 METRIC = "fp64 Mcell-substeps/s per RK3 step"
 UNIT = "Mcell-substeps/s"
 
@@ -82,6 +89,17 @@ def measured_peak_gbs():
         return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
+def cpu_model():
+    try:
+        with open("/proc/cpuinfo") as fh:
+            for ln in fh:
+                if ln.lower().startswith("model name"):
+                    return ln.split(":", 1)[1].strip()
+    except Exception:
+        pass
+    return "unknown"
+
+
 class ClockSampler(threading.Thread):
     """nvidia-smi clocks / throttle reasons sampled DURING the timed region."""
 
@@ -122,7 +140,7 @@ def run_reference(args, rank):
         return
     import oracle
     oracle.build()
-    n = args.ref_grid
+    n = args.cpu_grid
     cfg, f, dt, _ = W.make(args.workload, grid=(n, n, n), ndrops=max(1, 200 // (512 // n) ** 3))
     o = oracle.Oracle(cfg)
     o.set_fields(**f)
@@ -140,7 +158,7 @@ def run_reference(args, rank):
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": W.NAMES[args.workload], "sample": sample},
             "cpu_baseline": {"value": value, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
-                             "sample": sample},
+                             "cpu_model": cpu_model(), "sample": sample},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line), flush=True)
@@ -159,7 +177,79 @@ def cpu_baseline(args):
     el = time.perf_counter() - t0
     o.close()
     return {"value": n ** 3 * 3 / el / 1e6, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
-            "sample": "config %d recipe at %d^3, 1 RK3 step, %.1f s" % (args.workload, n, el)}
+            "cpu_model": cpu_model(), "sample": "config %d recipe at %d^3, 1 RK3 step, %.1f s" % (args.workload, n, el)}
+
+
+def cufft_compare(torch, cfg, per_kernel, device):
+    """Bench-only yardstick (BASELINE.json:5 "cuFFT appears only as a bench comparison"): the four transforms of S4
+    -- r2c along x, c2c along y, and their inverses -- by cuFFT through torch.fft on an array of the same shape,
+    plans created in a warm-up call.  The library's own S4 kernels additionally assemble the Poisson right-hand
+    side, solve the tridiagonal systems in z, scale and remove the gauge mean."""
+    try:
+        nz, ny, nx = cfg["nz"], cfg["ny"], cfg["nx"]
+        x = torch.randn(nz, ny, nx, dtype=torch.float64, device=device)
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(5)]
+
+        def run():
+            ev[0].record()
+            a = torch.fft.rfft(x, dim=2)
+            ev[1].record()
+            b = torch.fft.fft(a, dim=1)
+            ev[2].record()
+            c = torch.fft.ifft(b, dim=1)
+            ev[3].record()
+            d = torch.fft.irfft(c, n=nx, dim=2)
+            ev[4].record()
+            return d
+
+        run()
+        torch.cuda.synchronize()
+        best = [1e30] * 4
+        for _ in range(3):
+            run()
+            torch.cuda.synchronize()
+            best = [min(best[q], ev[q].elapsed_time(ev[q + 1])) for q in range(4)]
+        del x
+        torch.cuda.empty_cache()
+        ours = {k: per_kernel[k][0] / per_kernel[k][1] for k in ("k_fftx_fwd", "k_spec_fwd", "k_spec_bwd", "k_fftx_inv")
+                if k in per_kernel and per_kernel[k][1]}
+        return {"cufft_ms": {"rfft_x": round(best[0], 4), "fft_y": round(best[1], 4), "ifft_y": round(best[2], 4),
+                             "irfft_x": round(best[3], 4), "sum": round(sum(best), 4)},
+                "fizzy_s4_ms": {**{k: round(v, 4) for k, v in ours.items()}, "sum": round(sum(ours.values()), 4)},
+                "note": "cuFFT: transforms only, out of place, each a separate pass over HBM; fizzy S4: Poisson rhs + "
+                        "FFT x + (FFT y fused with the z tridiagonal sweeps) + inverse, scale, gauge"}
+    except Exception as exc:  # bench-only: never fail the line because of the yardstick
+        return {"error": repr(exc)}
+
+
+def graph_compare(torch, Fizzy, device):
+    """ms per RK3 step on the two launch-bound configurations (configs[0] 32^3, configs[1] 128^3)
+    with the three substeps as plain launches and replayed as one CUDA graph (fizzy_graph_enable)."""
+    out = {}
+    try:
+        for idx, steps in ((0, 200), (1, 50)):
+            cfg, f, dt, _ = W.make(idx)
+            row = {}
+            for mode in ("plain", "graph"):
+                st = torch.cuda.Stream(device)
+                g = Fizzy(cfg, stream=st, device=device)
+                g.fizzy_graph_enable(mode == "graph")
+                g.set_fields_numpy(**f)
+                for _ in range(10):
+                    g.fizzy_rk3_step(dt)
+                st.synchronize()
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record(st)
+                for _ in range(steps):
+                    g.fizzy_rk3_step(dt)
+                e1.record(st)
+                st.synchronize()
+                row[mode + "_ms_per_step"] = round(e0.elapsed_time(e1) / steps, 4)
+                g.close()
+            out[cfg["name"]] = row
+    except Exception as exc:
+        out["error"] = repr(exc)
+    return out
 
 
 def main():
@@ -170,8 +260,8 @@ def main():
     ap.add_argument("--workload", type=int, default=3, help="BASELINE.json config index (0-based)")
     ap.add_argument("--grid", type=int, nargs=3, default=None, help="override nx ny nz (debug)")
     ap.add_argument("--impl", default="fizzy", choices=["fizzy", "reference"])
-    ap.add_argument("--cpu-grid", type=int, default=256)
-    ap.add_argument("--ref-grid", type=int, default=128)
+    ap.add_argument("--cpu-grid", type=int, default=256, help="oracle sample grid (cpu_baseline and --impl reference)")
+    ap.add_argument("--no-cufft", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()
@@ -180,6 +270,14 @@ def main():
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        # `python bench.py --gpus N` without torchrun: start the N replicas ourselves (one rank per GPU)
+        cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(args.gpus),
+               "--master-addr", "127.0.0.1", "--master-port", os.environ.get("MASTER_PORT", "29511"),
+               os.path.abspath(__file__)] + sys.argv[1:]
+        os.execv(sys.executable, cmd)
+    if args.gpus != world:
+        raise SystemExit("bench.py: --gpus %d but WORLD_SIZE=%d" % (args.gpus, world))
 
     if args.impl == "reference":
         run_reference(args, rank)
@@ -210,11 +308,10 @@ def main():
             dist.barrier()
             torch.cuda.synchronize()
 
-    # ---------------- device-resident throughput (value) ----------------
+    # ---------------- device-resident throughput (value): per-kernel timing OFF ----------------
     for _ in range(args.warmup):
         fz.step(dt)
-    fz.fizzy_timing_enable(True)
-    fz.fizzy_timing_get(reset=True)
+    fz.fizzy_timing_enable(False)
     barrier()
     sampler = ClockSampler(local_rank)
     sampler.start()
@@ -229,14 +326,18 @@ def main():
     sampler.join()
     ms = e0.elapsed_time(e1)
     launches = fz.fizzy_launch_count() - n0
-    per_kernel = fz.fizzy_timing_get(reset=True)
-    fz.fizzy_timing_enable(False)
-    chk = torch.empty_like(dev["phi"])
-    fz.fizzy_get_fields(phi=chk)
-    torch.cuda.synchronize()
-    finite = bool(torch.isfinite(chk).all().item())
+    finite = fz.fizzy_check_finite() == 0
     ms = max_over_ranks(ms, dist, "cuda")
     value = whole_job_value(world, cells, 3 * args.steps, ms)
+
+    # ---------------- second pass, per-kernel events ON: the kernel table (not part of `value`) ----------------
+    ksteps = max(1, min(args.steps, 5))
+    fz.fizzy_timing_enable(True)
+    fz.fizzy_timing_get(reset=True)
+    for _ in range(ksteps):
+        fz.step(dt)
+    per_kernel = fz.fizzy_timing_get(reset=True)
+    fz.fizzy_timing_enable(False)
 
     # ---------------- roofline of the dominant kernel + per-kernel table ----------------
     peak, peak_src = measured_peak_gbs()
@@ -260,13 +361,15 @@ def main():
     if top:
         roofline = {"bound": "hbm", "kernel": top["kernel"], "achieved": top["achieved_GBs"], "peak": peak,
                     "unit": "GB/s", "frac": top["frac"], "traffic": None, "peak_source": peak_src}
-    # ncu DRAM traffic per launch of the dominant kernel, from the committed summary profiles/traffic.csv
+    # ncu DRAM traffic per launch of the dominant kernel: NOT measured in this run (a number printed under a
+    # profiler is never a bench value); it is the committed ncu capture named in `traffic_source`
     try:
-        with open(os.path.join(ROOT, "profiles", "traffic.csv")) as fh:
+        with open(os.path.join(ROOT, "profiles", TRAFFIC_CSV)) as fh:
             for ln in fh:
                 parts = ln.strip().split(",")
                 if roofline and len(parts) == 3 and parts[0] == cfg["name"] and parts[1] == roofline["kernel"]:
                     roofline["traffic"] = float(parts[2])
+                    roofline["traffic_source"] = "ncu --set full capture, profiles/%s (see profiles/%s)" % (TRAFFIC_CSV, TRAFFIC_MD)
     except Exception:
         pass
 
@@ -294,6 +397,10 @@ def main():
                "h2d_bytes_per_step": nb * len(names), "d2h_bytes_per_step": nb * len(names), "steps": ke,
                "note": "fizzy_set_fields(host) + 3 x fizzy_rk3_substep + fizzy_get_fields(host) per step"}
 
+    cufft = None
+    if rank == 0 and not args.no_cufft:
+        cufft = cufft_compare(torch, cfg, per_kernel, "cuda:%d" % local_rank)
+    graphs = graph_compare(torch, Fizzy, "cuda:%d" % local_rank) if (rank == 0 and world == 1 and not args.no_cufft) else None
     if rank != 0:
         if dist is not None:
             dist.destroy_process_group()
@@ -308,13 +415,17 @@ def main():
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": cfg["name"], "grid": [cfg["nx"], cfg["ny"], cfg["nz"]], "dt": dt,
                        "cache": "inputs larger than L2 (each field %.0f MB, 126 MB L2)" % (cells * 8 / 1e6),
-                       "parallelism": "replicas x%d" % world, "finite": finite},
+                       "parallelism": "replicas x%d" % world, "finite": finite,
+                       "byte_model": "SURVEY.md 8(d): %.0f B/cell/substep, every substep counted in full (stage 0 reads no RK "
+                                     "history and stage 2 writes none: those discounts are NOT taken)" % substep_model_bytes(cfg),
+                       "timing": "value: CUDA events on the library stream, per-kernel timing off; kernel table: second pass of "
+                                 "%d steps with events around every launch" % ksteps},
             "clocks": sampler.summary(), "e2e": e2e, "gpu_launches": launches,
             "roofline": roofline,
             "roofline_substep": {"bound": "hbm", "model_B_per_cell": substep_model_bytes(cfg),
                                  "ms_per_substep": sub_ms, "achieved": round(sub_gbs, 1), "peak": peak,
                                  "unit": "GB/s", "frac": round(sub_gbs / peak, 4)},
-            "kernels": table, "cpu_baseline": cpu}
+            "kernels": table, "cufft_compare": cufft, "graph_compare": graphs, "cpu_baseline": cpu}
     print(json.dumps(line), flush=True)
     if dist is not None:
         dist.destroy_process_group()

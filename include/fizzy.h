@@ -83,11 +83,15 @@ typedef struct {
 /* Bytes of device workspace fizzy_create needs for this grid / property set (0 on bad input). */
 size_t fizzy_workspace_bytes(const fizzy_grid *grid, const fizzy_bc *bc, const fizzy_props *props);
 
-/* Create a context.  `dev_workspace` must hold at least fizzy_workspace_bytes() bytes, be
+/* Create a context for one grid / boundary set / fluid pair (3-D Cartesian grid, staggered
+ * velocity, cell-centred scalars; two fluids with properties mapped over phi; BASELINE.json:7-11 for
+ * the boundary sets: x, y periodic, z periodic or walls, uniform or stretched).  `dev_workspace` must hold at least fizzy_workspace_bytes() bytes, be
  * 256-byte aligned and outlive the context.  `cuda_stream` is a cudaStream_t (NULL = default
  * stream).  Builds the 1-D metric tables, FFT twiddles, modified wavenumbers
  * lam_x(l) = -4 sin^2(pi l/nx)/dx^2 (lam_y likewise) and the z-tridiagonal elimination tables.
- * FIZZY_EINVAL: nx, ny not powers of two in [8,1024], nz < 4, nx*ny*nz >= 2^31, lengths <= 0, non-monotone zf,
+ * The workspace must be memory of the CUDA device that is current at this call; every later call on the context
+ * must find the same device current (FIZZY_ESTATE otherwise).
+ * FIZZY_EINVAL: nx, ny not powers of two in [8,1024], nz < 4 or > 65535, nx*ny*nz >= 2^31, lengths <= 0, non-monotone zf,
  * zf given with z_wall = 0, rho <= 0, mu < 0, eps <= 0, delta < 1e-150, cp or kth <= 0 with heat on,
  * misaligned workspace.  FIZZY_ENOMEM: workspace too small. */
 fizzy_status fizzy_create(const fizzy_grid *grid, const fizzy_bc *bc, const fizzy_props *props,
@@ -96,7 +100,9 @@ fizzy_status fizzy_create(const fizzy_grid *grid, const fizzy_bc *bc, const fizz
 
 fizzy_status fizzy_destroy(fizzy_ctx *ctx);
 
-/* Load the prognostic fields (host or device pointers, N doubles each).  NULL = leave unchanged
+/* Load the prognostic fields of the one-fluid model (velocity, pressure, phase indicator phi,
+ * temperature; p_prev is the previous substep pressure of the splitting, N7) in the layout above (PAPER.md:36
+ * staggered arrangement).  Host or device pointers, N doubles each.  NULL = leave unchanged
  * (the workspace starts zero-filled).  p_prev == NULL sets p_prev := p when p is given.
  * Zeroes the RK history, enforces w[:,:,nz-1] = 0 with walls, recomputes max|u| and the
  * interface quantities of phi, and resets the stage counter to 0. */
@@ -111,27 +117,52 @@ fizzy_status fizzy_set_fields(fizzy_ctx *ctx, const double *u, const double *v, 
  * FIZZY_EINVAL: stage not in {0,1,2} or dt <= 0.  FIZZY_ESTATE: fields not set / wrong stage. */
 fizzy_status fizzy_rk3_substep(fizzy_ctx *ctx, int stage, double dt);
 
+/* One full RK3 step = the three substeps above in order ("low-storage three-step Runge-Kutta").
+ * With fizzy_graph_enable(ctx, 1) the three substeps (about 25 kernel launches) are captured once into a CUDA
+ * graph per buffer rotation and time step and replayed afterwards -- what matters on the 32^3 .. 128^3
+ * configurations, where a substep is launch-bound.  The results are bit-identical to the
+ * plain launches.  Graph capture needs a context created on a non-default stream (FIZZY_EINVAL otherwise) and
+ * is bypassed while fizzy_timing_enable is on.  FIZZY_ESTATE unless the next stage is 0. */
+fizzy_status fizzy_rk3_step(fizzy_ctx *ctx, double dt);
+fizzy_status fizzy_graph_enable(fizzy_ctx *ctx, int on);
+
+/* Stable time step of the CURRENT fields, reading N16 of DESIGN.md (BASELINE.json:8 "dt from CFL 0.5"):
+ *   dt = cfl * min( 1/max(|u|/dx + |v|/dy + |w|/dzf),  1/(2 nu_max S),  sqrt((rho1+rho2) dmin^3/(4 pi sigma)),
+ *                   1/(2 Gamma eps S),  1/(2 a_max S) [heat on] ),   S = 1/dx^2 + 1/dy^2 + 1/dzmin^2,
+ * Gamma = gamma_rel*max|u| + gamma_abs.  The two maxima are reduced on the device (one pass over u, v, w); the
+ * scalar formula is evaluated on the host.  Synchronises the stream.  *dt = 0 if nothing limits.
+ * FIZZY_EINVAL: dt NULL or cfl <= 0.  FIZZY_ESTATE before fizzy_set_fields. */
+fizzy_status fizzy_stable_dt(fizzy_ctx *ctx, double cfl, double *dt);
+
+/* Number of non-finite values among u, v, w, p, phi (and T with heat on); one pass, synchronises the stream. */
+fizzy_status fizzy_check_finite(fizzy_ctx *ctx, long long *count);
+
 /* Solve Lap p = rhs with the context's grid and z boundary condition (periodic x, y; periodic
  * or homogeneous Neumann z): FFT in x and y, tridiagonal in z (BASELINE.json:5(iv)).  The
  * singular mean mode follows N17: last row replaced by p_hat(nz-1) = 0, then the dzf-weighted
  * mean is removed.  rhs and p are N doubles, host or device; they may alias. */
 fizzy_status fizzy_poisson_solve(fizzy_ctx *ctx, const double *rhs, double *p);
 
-/* Copy fields out (host or device pointers); any pointer may be NULL. */
+/* Copy the prognostic fields out (same layout and meaning as fizzy_set_fields; host or device pointers); any
+ * pointer may be NULL.  Enqueued on the stream like every other call: synchronise before reading host memory. */
 fizzy_status fizzy_get_fields(fizzy_ctx *ctx, double *u, double *v, double *w, double *p,
                               double *phi, double *T, double *p_prev);
 
 /* Run-time diagnostics of the current state (definitions in DESIGN.md 10), one pass
- * over the fields and a fixed-order (deterministic) reduction.  `out` = 6 HOST doubles, dV = dx*dy*dzf[k]:
+ * over the fields and a fixed-order (deterministic) reduction.  `out` = 8 HOST doubles, dV = dx*dy*dzf[k]:
  *   out[0] = sum phi dV (volume of fluid 1)        out[1] = 1/2 sum rho(phi) |u_c|^2 dV, u_c = cell-centred mean
  *   out[2] = max over faces of max(|u|,|v|,|w|)    out[3] = max |D(u)|
  *   out[4] = sum |grad phi| dV (central differences: area of the diffuse interface)
- *   out[5] = sum T dV / sum dV (0 with heat off).
+ *   out[5] = sum T dV / sum dV (0 with heat off)
+ *   out[6], out[7] = Nusselt number at the bottom, top wall: <-dT/dz>_wall * lz/(t_wall[0] - t_wall[1]), the wall
+ *            gradient taken through the Dirichlet ghost 2 T_wall - T (0 unless heat on, z_wall = 1, t_wall differ).
  * Synchronises the stream.  FIZZY_ESTATE before fizzy_set_fields. */
 fizzy_status fizzy_diagnostics(fizzy_ctx *ctx, double *out);
 
-/* Current Gamma (synchronises the stream).  NaN if ctx is NULL. */
-double fizzy_gamma(fizzy_ctx *ctx);
+/* Current Gamma = gamma_rel*max|u| + gamma_abs as latched at the last stage 0 (N15; BASELINE.json:8-11
+ * "Gamma = max|u|"); gamma_abs before the first substep.  Synchronises the stream.  NaN if ctx is NULL or
+ * its device is not current. */
+double fizzy_gamma(const fizzy_ctx *ctx);
 
 /* Number of kernels the library has launched on this context so far (host counter). */
 long long fizzy_launch_count(const fizzy_ctx *ctx);

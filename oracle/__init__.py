@@ -70,6 +70,8 @@ def _load():
         lib.orc_substep.restype = C.c_int
         lib.orc_poisson_solve.argtypes = [C.c_void_p, _dp, _dp]
         lib.orc_diagnostics.argtypes = [C.c_void_p, _dp]
+        lib.orc_stable_dt.argtypes = [C.c_void_p, C.c_double]
+        lib.orc_stable_dt.restype = C.c_double
         lib.orc_gamma.argtypes = [C.c_void_p]
         lib.orc_gamma.restype = C.c_double
         lib.orc_get_intermediate.argtypes = [C.c_void_p, C.c_char_p, _dp]
@@ -157,10 +159,14 @@ class Oracle:
         return out
 
     def diagnostics(self) -> np.ndarray:
-        """[volume of fluid 1, kinetic energy, max|u|, max|D(u)|, interfacial area, mean T]"""
-        out = np.zeros(6)
+        """[volume of fluid 1, kinetic energy, max|u|, max|D(u)|, interfacial area, mean T, Nu bottom, Nu top]"""
+        out = np.zeros(8)
         _load().orc_diagnostics(self._h, out.ctypes.data_as(_dp))
         return out
+
+    def stable_dt(self, cfl: float = 0.5) -> float:
+        """N16: cfl * min(advective, viscous, capillary, ACDI, thermal limit) of the current fields."""
+        return float(_load().orc_stable_dt(self._h, float(cfl)))
 
     def gamma(self) -> float:
         return float(_load().orc_gamma(self._h))

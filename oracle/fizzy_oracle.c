@@ -913,6 +913,9 @@ int orc_get_intermediate(const orc_state *st, const char *name, double *out)
  *   out[4] = sum |grad phi| dV, central differences (phi(+1_a) - phi(-1_a))/(hc_a + hc_a(-1_a))
  *            (interfacial area of a diffuse interface)
  *   out[5] = sum T dV / sum dV   (0 if heat is off)
+ *   out[6], out[7] = Nusselt number at the bottom / top wall (heat on, walls, t_bot != t_top; else 0):
+ *            Nu = <-dT/dz>_wall * lz / (t_bot - t_top), the wall gradient taken through the Dirichlet
+ *            ghost T(-1) = 2 T_wall - T(0) at distance dzf[0]  (SURVEY.md 8(c) "Walls")
  * Ghosts of u, v, w, phi, T are up to date after orc_set_fields / orc_substep. */
 void orc_diagnostics(const orc_state *st, double *out)
 {
@@ -944,4 +947,51 @@ void orc_diagnostics(const orc_state *st, double *out)
             }
     out[0] = vol1; out[1] = ke; out[2] = umax; out[3] = dmax; out[4] = area;
     out[5] = st->P.heat ? tsum / vsum : 0.0;
+    out[6] = out[7] = 0.0;
+    if (st->P.heat && st->P.z_wall && st->P.t_bot != st->P.t_top) {
+        double gb = 0.0, gt = 0.0;   /* sum over the wall of -dT/dz */
+        for (int j = 0; j < ny; ++j)
+            for (int i = 0; i < nx; ++i) {
+                gb += -(st->T[IDX(i, j, 0)] - st->T[IDX(i, j, -1)]) / DZC(-1);
+                gt += -(st->T[IDX(i, j, nz)] - st->T[IDX(i, j, nz - 1)]) / DZC(nz - 1);
+            }
+        const double scale = st->P.lz / (st->P.t_bot - st->P.t_top) / ((double)nx * ny);
+        out[6] = gb * scale;
+        out[7] = gt * scale;
+    }
+}
+
+/* ------------------------------------------------------------------ stable time step (N16)
+ * dt = cfl * min(dt_adv, dt_visc, dt_sigma, dt_acdi, dt_heat) of the CURRENT fields:
+ *   dt_adv   = 1 / max over cells of (|u|/dx + |v|/dy + |w|/dzf[k])   (face values of the same index)
+ *   dt_visc  = 1 / (2 nu_max S),   nu_max = max(mu1/rho1, mu2/rho2),  S = 1/dx^2 + 1/dy^2 + 1/dzmin^2
+ *   dt_sigma = sqrt((rho1 + rho2) dmin^3 / (4 pi sigma)),             dmin = min(dx, dy, dzmin)
+ *   dt_acdi  = 1 / (2 Gamma eps S),  Gamma = gamma_rel * max(|u|,|v|,|w|) + gamma_abs   (N15)
+ *   dt_heat  = 1 / (2 a_max S),    a_max = max(k1/(rho1 cp1), k2/(rho2 cp2))            (heat on)
+ * a limit whose denominator vanishes is left out; returns 0 if every limit is left out. */
+double orc_stable_dt(const orc_state *st, double cfl)
+{
+    const int nx = st->nx, ny = st->ny, nz = st->nz;
+    const orc_params *P = &st->P;
+    double adv = 0.0, umax = 0.0, dzmin = DZF(0);
+    for (int k = 0; k < nz; ++k) {
+        dzmin = fmin(dzmin, DZF(k));
+        for (int j = 0; j < ny; ++j)
+            for (int i = 0; i < nx; ++i) {
+                const size_t c = IDX(i, j, k);
+                adv = fmax(adv, fabs(st->u[c]) / st->dx + fabs(st->v[c]) / st->dy + fabs(st->w[c]) / DZF(k));
+                umax = fmax(umax, fmax(fabs(st->u[c]), fmax(fabs(st->v[c]), fabs(st->w[c]))));
+            }
+    }
+    const double S = 1.0 / (st->dx * st->dx) + 1.0 / (st->dy * st->dy) + 1.0 / (dzmin * dzmin);
+    const double dmin = fmin(st->dx, fmin(st->dy, dzmin));
+    const double gam = P->gamma_rel * umax + P->gamma_abs;
+    const double nu = fmax(P->mu1 / P->rho1, P->mu2 / P->rho2);
+    double lim = INFINITY;
+    if (adv > 0.0) lim = fmin(lim, 1.0 / adv);
+    if (nu > 0.0) lim = fmin(lim, 1.0 / (2.0 * nu * S));
+    if (P->sigma > 0.0) lim = fmin(lim, sqrt((P->rho1 + P->rho2) * dmin * dmin * dmin / (4.0 * M_PI * P->sigma)));
+    if (gam > 0.0) lim = fmin(lim, 1.0 / (2.0 * gam * P->eps * S));
+    if (P->heat) lim = fmin(lim, 1.0 / (2.0 * fmax(P->k1 / (P->rho1 * P->cp1), P->k2 / (P->rho2 * P->cp2)) * S));
+    return isinf(lim) ? 0.0 : cfl * lim;
 }

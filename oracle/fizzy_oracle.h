@@ -85,9 +85,14 @@ void orc_temperature_rhs(orc_state *st, double *rhs_T);
  * in-place, n a power of two, sign=-1 forward (e^{-2 pi i jk/n}), +1 backward (no scaling) */
 void orc_fft(int n, double *re, double *im, int sign);
 
-/* run-time diagnostics of the current state: out[6] = volume of fluid 1,
- * kinetic energy, max|u|, max|D(u)|, interfacial area, mean temperature (see fizzy_oracle.c) */
+/* run-time diagnostics of the current state: out[8] = volume of fluid 1,
+ * kinetic energy, max|u|, max|D(u)|, interfacial area, mean temperature, Nusselt number at the
+ * bottom and at the top wall (see fizzy_oracle.c) */
 void orc_diagnostics(const orc_state *st, double *out);
+
+/* stable time step of the current fields, reading N16: cfl * min of the advective,
+ * viscous, capillary, ACDI and thermal limits (see fizzy_oracle.c) */
+double orc_stable_dt(const orc_state *st, double cfl);
 
 int orc_num_threads(void);
 

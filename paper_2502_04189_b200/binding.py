@@ -18,7 +18,8 @@ _STATUS = {0: "FIZZY_OK", 1: "FIZZY_EINVAL", 2: "FIZZY_ENOMEM", 3: "FIZZY_ECUDA"
 
 EXPORTS = ["fizzy_workspace_bytes", "fizzy_create", "fizzy_destroy", "fizzy_set_fields",
            "fizzy_rk3_substep", "fizzy_poisson_solve", "fizzy_get_fields", "fizzy_gamma", "fizzy_diagnostics",
-           "fizzy_launch_count", "fizzy_last_error", "fizzy_timing_enable", "fizzy_timing_get"]
+           "fizzy_launch_count", "fizzy_last_error", "fizzy_timing_enable", "fizzy_timing_get",
+           "fizzy_rk3_step", "fizzy_graph_enable", "fizzy_stable_dt", "fizzy_check_finite"]
 
 
 class FizzyGrid(C.Structure):
@@ -69,6 +70,14 @@ def load_library(path: str = LIB_PATH) -> C.CDLL:
     lib.fizzy_poisson_solve.argtypes = [vp, dp, dp]
     lib.fizzy_diagnostics.restype = C.c_int
     lib.fizzy_diagnostics.argtypes = [vp, C.POINTER(C.c_double)]
+    lib.fizzy_rk3_step.restype = C.c_int
+    lib.fizzy_rk3_step.argtypes = [vp, C.c_double]
+    lib.fizzy_graph_enable.restype = C.c_int
+    lib.fizzy_graph_enable.argtypes = [vp, C.c_int]
+    lib.fizzy_stable_dt.restype = C.c_int
+    lib.fizzy_stable_dt.argtypes = [vp, C.c_double, C.POINTER(C.c_double)]
+    lib.fizzy_check_finite.restype = C.c_int
+    lib.fizzy_check_finite.argtypes = [vp, C.POINTER(C.c_longlong)]
     lib.fizzy_gamma.restype = C.c_double
     lib.fizzy_gamma.argtypes = [vp]
     lib.fizzy_launch_count.restype = C.c_longlong
@@ -145,15 +154,22 @@ class Fizzy:
         if nbytes == 0:
             raise FizzyError(FIZZY_EINVAL, "invalid grid / bc / props")
         self.workspace_bytes = nbytes
+        if self.device.index is None:
+            self.device = torch.device("cuda", torch.cuda.current_device())
         self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
         base = self.workspace.data_ptr()
         aligned = (base + 255) & ~255
         self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
         h = C.c_void_p()
-        st = _lib.fizzy_create(C.byref(g), C.byref(bc), C.byref(pr), aligned, nbytes,
-                               self.stream.cuda_stream, C.byref(h))
+        with torch.cuda.device(self.device):
+            st = _lib.fizzy_create(C.byref(g), C.byref(bc), C.byref(pr), aligned, nbytes,
+                                   self.stream.cuda_stream, C.byref(h))
         self._h = h if h.value else None
         self._check(st)
+
+    def _on_device(self):
+        """The library launches on the CURRENT device: make the context's device current around every call."""
+        return self._torch.cuda.device(self.device)
 
     def _check(self, st):
         if st != FIZZY_OK:
@@ -162,31 +178,57 @@ class Fizzy:
 
     def close(self):
         if getattr(self, "_h", None):
-            _lib.fizzy_destroy(self._h)
+            with self._on_device():
+                _lib.fizzy_destroy(self._h)
             self._h = None
 
     __del__ = close
 
     # ---- the C-ABI calls, same names ----
     def fizzy_set_fields(self, u=None, v=None, w=None, p=None, phi=None, T=None, p_prev=None):
-        self._check(_lib.fizzy_set_fields(self._h, *[_addr(a) for a in (u, v, w, p, phi, T, p_prev)]))
+        with self._on_device():
+            self._check(_lib.fizzy_set_fields(self._h, *[_addr(a) for a in (u, v, w, p, phi, T, p_prev)]))
 
     def fizzy_get_fields(self, u=None, v=None, w=None, p=None, phi=None, T=None, p_prev=None):
-        self._check(_lib.fizzy_get_fields(self._h, *[_addr(a) for a in (u, v, w, p, phi, T, p_prev)]))
+        with self._on_device():
+            self._check(_lib.fizzy_get_fields(self._h, *[_addr(a) for a in (u, v, w, p, phi, T, p_prev)]))
 
     def fizzy_rk3_substep(self, stage: int, dt: float):
-        self._check(_lib.fizzy_rk3_substep(self._h, int(stage), float(dt)))
+        with self._on_device():
+            self._check(_lib.fizzy_rk3_substep(self._h, int(stage), float(dt)))
 
     def fizzy_poisson_solve(self, rhs, p):
-        self._check(_lib.fizzy_poisson_solve(self._h, _addr(rhs), _addr(p)))
+        with self._on_device():
+            self._check(_lib.fizzy_poisson_solve(self._h, _addr(rhs), _addr(p)))
 
     def fizzy_diagnostics(self) -> np.ndarray:
-        out = (C.c_double * 6)()
-        self._check(_lib.fizzy_diagnostics(self._h, out))
+        out = (C.c_double * 8)()
+        with self._on_device():
+            self._check(_lib.fizzy_diagnostics(self._h, out))
         return np.array(out[:])
 
+    def fizzy_rk3_step(self, dt: float):
+        with self._on_device():
+            self._check(_lib.fizzy_rk3_step(self._h, float(dt)))
+
+    def fizzy_graph_enable(self, on: bool):
+        self._check(_lib.fizzy_graph_enable(self._h, int(bool(on))))
+
+    def fizzy_stable_dt(self, cfl: float = 0.5) -> float:
+        dt = C.c_double()
+        with self._on_device():
+            self._check(_lib.fizzy_stable_dt(self._h, float(cfl), C.byref(dt)))
+        return dt.value
+
+    def fizzy_check_finite(self) -> int:
+        n = C.c_longlong()
+        with self._on_device():
+            self._check(_lib.fizzy_check_finite(self._h, C.byref(n)))
+        return n.value
+
     def fizzy_gamma(self) -> float:
-        return float(_lib.fizzy_gamma(self._h))
+        with self._on_device():
+            return float(_lib.fizzy_gamma(self._h))
 
     def fizzy_launch_count(self) -> int:
         return int(_lib.fizzy_launch_count(self._h))
@@ -208,8 +250,7 @@ class Fizzy:
 
     # ---- conveniences (marshalling only) ----
     def step(self, dt: float):
-        for s in range(3):
-            self.fizzy_rk3_substep(s, dt)
+        self.fizzy_rk3_step(dt)
 
     def set_fields_numpy(self, **f):
         self.fizzy_set_fields(**{k: np.ascontiguousarray(a, dtype=np.float64) for k, a in f.items()})

@@ -54,6 +54,7 @@ struct fizzy_ctx {
     double t_ms[FZK_COUNT] = {0};
     long long t_n[FZK_COUNT] = {0};
     cudaStream_t stream;
+    int device;                // CUDA device the context was created on (every later call must find it current)
     bool varrho, varmu, heat, cyclic;
     int log2nx, log2ny;
     long long N, M;
@@ -65,7 +66,16 @@ struct fizzy_ctx {
     double *kappa, *divrn, *psi, *rr, *nhx, *nhy, *nhz, *rnx, *rny, *rnz;
     double2 *spec;
     double2 *twx, *twy;
-    double *scal;  // [0] running max|u|, [1] Gamma, [2] gauge mean, [8..13] diagnostics
+    double *scal;  // [0] running max|u|, [1] Gamma, [2] gauge mean, [3..4] dt maxima, [5] non-finite count, [8..15] diagnostics
+    double dzmin;  // smallest cell height (N16)
+    // one RK3 step as a CUDA graph (fizzy_graph_enable): one executable graph per parity of the step counter,
+    // because phi/phi_new (and T/T_new) swap three times per step and are back in place after two steps
+    bool graph_on = false;
+    double *phi0 = nullptr;                       // the buffer phi occupied at creation: selects the graph slot
+    cudaGraphExec_t gexec[2] = {nullptr, nullptr};
+    double gdt[2] = {0.0, 0.0};
+    const double *gkey[2][2] = {{nullptr, nullptr}, {nullptr, nullptr}};   // p, p_prev buffers baked into the graph
+    long long glaunches[2] = {0, 0};
     double *dpart; // block partials of k_diag
     FzTri tri;
     int fields_set, next_stage;
@@ -82,7 +92,7 @@ bool valid_inputs(const fizzy_grid *g, const fizzy_bc *bc, const fizzy_props *pr
 {
     if (!g || !bc || !pr) return false;
     if (!is_pow2(g->nx) || !is_pow2(g->ny) || g->nx < 8 || g->ny < 8 || g->nx > 1024 || g->ny > 1024) return false;
-    if (g->nz < 4) return false;
+    if (g->nz < 4 || g->nz > 65535) return false;                          // k rides in gridDim.z
     if ((long long)g->nx * g->ny * g->nz >= (1LL << 31)) return false;   // kernels use 32-bit cell offsets
     if (!(g->lx > 0) || !(g->ly > 0) || !(g->lz > 0)) return false;
     if (bc->z_wall != 0 && bc->z_wall != 1) return false;
@@ -177,6 +187,8 @@ cudaEvent_t take_event(fizzy_ctx *c)
         if (e_ != cudaSuccess) return cuda_fail(c, e_, FZK_NAME[id_]);  \
     } while (0)
 
+cudaError_t launch_momentum(fizzy_ctx *c, dim3 grid, dim3 block, const FzMomArgs *A);   // defined with the substep
+
 void cell_launch(const fizzy_ctx *c, dim3 &grid, dim3 &block)
 {
     const int bx = c->P.nx < 64 ? c->P.nx : 64;
@@ -210,6 +222,15 @@ extern "C" fizzy_status fizzy_create(const fizzy_grid *grid, const fizzy_bc *bc,
     if (!c) return FIZZY_ENOMEM;
     *out = c;  // returned even on a CUDA failure below so that fizzy_last_error can be read
     c->stream = static_cast<cudaStream_t>(cuda_stream);
+    FZ_CUDA(cudaGetDevice(&c->device));
+    {   // the workspace must live on the current device
+        cudaPointerAttributes pa;
+        if (cudaPointerGetAttributes(&pa, dev_workspace) != cudaSuccess || pa.type != cudaMemoryTypeDevice ||
+            pa.device != c->device) {
+            cudaGetLastError();
+            return fail(c, FIZZY_EINVAL, "dev_workspace is not device memory of the current CUDA device");
+        }
+    }
     c->fields_set = 0;
     c->next_stage = 0;
     c->launches = 0;
@@ -217,6 +238,7 @@ extern "C" fizzy_status fizzy_create(const fizzy_grid *grid, const fizzy_bc *bc,
     const int nx = grid->nx, ny = grid->ny, nz = grid->nz;
     double *ztab[5], *acoef[2], *lam[2];
     const size_t used = layout(c, dev_workspace, grid, bc, props, ztab, acoef, lam);
+    c->phi0 = c->phi;
     FZ_CUDA(cudaMemsetAsync(dev_workspace, 0, used, c->stream));
 
     FzP &P = c->P;
@@ -225,7 +247,7 @@ extern "C" fizzy_status fizzy_create(const fizzy_grid *grid, const fizzy_bc *bc,
     P.z_wall = bc->z_wall; P.heat = props->heat ? 1 : 0;
     P.kzf = bc->z_wall ? nz - 1 : nz;
     P.N = (long long)nx * ny * nz; P.sxy = (long long)nx * ny;
-    P.dx = grid->lx / nx; P.dy = grid->ly / ny; P.idx = 1.0 / P.dx; P.idy = 1.0 / P.dy;
+    P.dx = grid->lx / nx; P.dy = grid->ly / ny; P.idx = 1.0 / P.dx; P.idy = 1.0 / P.dy; P.lz = grid->lz;
     P.rho1 = props->rho[0]; P.rho2 = props->rho[1]; P.mu1 = props->mu[0]; P.mu2 = props->mu[1];
     P.k1 = props->kth[0]; P.k2 = props->kth[1]; P.cp1 = props->cp[0]; P.cp2 = props->cp[1];
     P.sigma = props->sigma; P.eps = props->eps; P.delta = props->delta;
@@ -250,6 +272,8 @@ extern "C" fizzy_status fizzy_create(const fizzy_grid *grid, const fizzy_bc *bc,
     for (int q = 0; q < nzt - 1; ++q) dzc[q] = 0.5 * (dzf[q] + dzf[q + 1]);
     dzc[nzt - 1] = dzc[nzt - 2];
     for (int q = 0; q < nzt; ++q) { idzf[q] = 1.0 / dzf[q]; idzc[q] = 1.0 / dzc[q]; }
+    c->dzmin = dzf[FZ_H];
+    for (int k = 0; k < nz; ++k) c->dzmin = std::fmin(c->dzmin, dzf[k + FZ_H]);
     for (int q = 1; q < nzt; ++q) igz[q] = 1.0 / (dzc[q] + dzc[q - 1]);
     const std::vector<double> *tabs[5] = {&dzf, &dzc, &idzf, &idzc, &igz};
     for (int q = 0; q < 5; ++q)
@@ -283,9 +307,14 @@ extern "C" fizzy_status fizzy_create(const fizzy_grid *grid, const fizzy_bc *bc,
     k_tri_tables<<<(unsigned)((c->M + 127) / 128), 128, 0, c->stream>>>(P, c->tri);
     FZ_LAUNCHED(FZK_OTHER);
 
-    // dynamic shared memory opt-in (the FFT kernels opt in at launch, per instantiation)
+    // dynamic shared memory opt-in of every kernel instantiation this context will launch: once, here,
+    // so that a substep is launches only (and can be captured into a CUDA graph)
     FZ_CUDA(cudaFuncSetAttribute(k_iface_march<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)IFACE_SMEM));
     FZ_CUDA(cudaFuncSetAttribute(k_iface_march<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)IFACE_SMEM));
+    FZ_CUDA(launch_momentum(c, dim3(), dim3(), nullptr));
+    FZ_CUDA(fz_fftx_launch(-1, c->log2nx, P, nullptr, nullptr, nullptr, nullptr, 0.0, nullptr, nullptr, nullptr, nullptr, c->stream));
+    FZ_CUDA(c->cyclic ? fz_spec_launch<true>(-1, c->log2ny, P, c->tri, nullptr, nullptr, nullptr, c->stream)
+                      : fz_spec_launch<false>(-1, c->log2ny, P, c->tri, nullptr, nullptr, nullptr, c->stream));
     return FIZZY_OK;
 }
 
@@ -295,6 +324,8 @@ extern "C" fizzy_status fizzy_destroy(fizzy_ctx *c)
     cudaStreamSynchronize(c->stream);
     for (FzTimed &t : c->pending) { cudaEventDestroy(t.e0); cudaEventDestroy(t.e1); }
     for (cudaEvent_t e : c->pool) cudaEventDestroy(e);
+    for (cudaGraphExec_t g : c->gexec)
+        if (g) cudaGraphExecDestroy(g);
     delete c;
     return FIZZY_OK;
 }
@@ -330,9 +361,11 @@ extern "C" fizzy_status fizzy_timing_get(fizzy_ctx *c, int index, const char **n
 extern "C" const char *fizzy_last_error(const fizzy_ctx *c) { return c ? c->err.c_str() : "null context"; }
 extern "C" long long fizzy_launch_count(const fizzy_ctx *c) { return c ? c->launches : 0; }
 
-extern "C" double fizzy_gamma(fizzy_ctx *c)
+extern "C" double fizzy_gamma(const fizzy_ctx *c)
 {
     if (!c) return NAN;
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev != c->device) return NAN;
     double g = NAN;
     if (cudaMemcpyAsync(&g, c->scal + 1, sizeof(double), cudaMemcpyDeviceToHost, c->stream) != cudaSuccess) return NAN;
     if (cudaStreamSynchronize(c->stream) != cudaSuccess) return NAN;
@@ -394,12 +427,12 @@ fizzy_status run_spectral_solve(fizzy_ctx *c, double *dst)
 {
     const FzP &P = c->P;
     FZ_TB(FZK_SPEC_FWD);
-    FZ_CUDA(c->cyclic ? fz_spec_launch<true>(true, c->log2ny, P, c->tri, c->spec, c->twy, c->scal, c->stream)
-                      : fz_spec_launch<false>(true, c->log2ny, P, c->tri, c->spec, c->twy, c->scal, c->stream));
+    FZ_CUDA(c->cyclic ? fz_spec_launch<true>(0, c->log2ny, P, c->tri, c->spec, c->twy, c->scal, c->stream)
+                      : fz_spec_launch<false>(0, c->log2ny, P, c->tri, c->spec, c->twy, c->scal, c->stream));
     FZ_LAUNCHED(FZK_SPEC_FWD);
     FZ_TB(FZK_SPEC_BWD);
-    FZ_CUDA(c->cyclic ? fz_spec_launch<true>(false, c->log2ny, P, c->tri, c->spec, c->twy, c->scal, c->stream)
-                      : fz_spec_launch<false>(false, c->log2ny, P, c->tri, c->spec, c->twy, c->scal, c->stream));
+    FZ_CUDA(c->cyclic ? fz_spec_launch<true>(1, c->log2ny, P, c->tri, c->spec, c->twy, c->scal, c->stream)
+                      : fz_spec_launch<false>(1, c->log2ny, P, c->tri, c->spec, c->twy, c->scal, c->stream));
     FZ_LAUNCHED(FZK_SPEC_BWD);
     FZ_TB(FZK_FFTX_INV);
     FZ_CUDA(fz_fftx_launch(2, c->log2nx, P, nullptr, nullptr, nullptr, nullptr, 1.0 / ((double)P.nx * (double)P.ny),
@@ -408,14 +441,15 @@ fizzy_status run_spectral_solve(fizzy_ctx *c, double *dst)
     return FIZZY_OK;
 }
 
+// A == NULL: shared-memory opt-in of the variant this context uses (once, at fizzy_create)
 template <bool VR, bool VM, bool HT>
-cudaError_t launch_momentum3(fizzy_ctx *c, dim3 grid, dim3 block, const FzMomArgs &A)
+cudaError_t launch_momentum3(fizzy_ctx *c, dim3 grid, dim3 block, const FzMomArgs *Ap)
 {
     const FzP &P = c->P;
+    const size_t smem = (size_t)FzMomFields<VR, HT>::NF * MRING * MPS * sizeof(double);
+    if (!Ap) return cudaFuncSetAttribute(k_momentum_march<VR, VM, HT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    const FzMomArgs &A = *Ap;
     if (P.nx >= MTX && P.ny >= MTY) {   // 2.5-D marching kernel
-        const size_t smem = (size_t)FzMomFields<VR, HT>::NF * MRING * MPS * sizeof(double);
-        cudaError_t e = cudaFuncSetAttribute(k_momentum_march<VR, VM, HT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
         const int tiles = (P.nx / MTX) * (P.ny / MTY);
         int chunks = 8192 / tiles;
         if (chunks > P.nz / 16) chunks = P.nz / 16;
@@ -430,10 +464,30 @@ cudaError_t launch_momentum3(fizzy_ctx *c, dim3 grid, dim3 block, const FzMomArg
 }
 
 template <bool VR, bool VM>
-cudaError_t launch_momentum(fizzy_ctx *c, dim3 grid, dim3 block, const FzMomArgs &A)
+cudaError_t launch_momentum2(fizzy_ctx *c, dim3 grid, dim3 block, const FzMomArgs *A)
 {
     return c->heat ? launch_momentum3<VR, VM, true>(c, grid, block, A) : launch_momentum3<VR, VM, false>(c, grid, block, A);
 }
+
+cudaError_t launch_momentum(fizzy_ctx *c, dim3 grid, dim3 block, const FzMomArgs *A)
+{
+    if (c->varrho) return c->varmu ? launch_momentum2<true, true>(c, grid, block, A) : launch_momentum2<true, false>(c, grid, block, A);
+    return c->varmu ? launch_momentum2<false, true>(c, grid, block, A) : launch_momentum2<false, false>(c, grid, block, A);
+}
+
+// every entry point after fizzy_create: the context's device must be the current one
+fizzy_status check_device(fizzy_ctx *c)
+{
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev != c->device)
+        return fail(c, FIZZY_ESTATE, "the CUDA device the context was created on is not the current device");
+    return FIZZY_OK;
+}
+#define FZ_DEVICE()                                      \
+    do {                                                 \
+        const fizzy_status ds_ = check_device(c);        \
+        if (ds_ != FIZZY_OK) return ds_;                 \
+    } while (0)
 
 }  // namespace
 
@@ -442,6 +496,7 @@ extern "C" fizzy_status fizzy_set_fields(fizzy_ctx *c, const double *u, const do
                                          const double *p_prev)
 {
     if (!c) return FIZZY_EINVAL;
+    FZ_DEVICE();
     const size_t B = (size_t)c->N * sizeof(double);
     const double *src[] = {u, v, w, p, phi, c->heat ? T : nullptr};
     double *dst[] = {c->u, c->v, c->w, c->p, c->phi, c->T};
@@ -457,9 +512,9 @@ extern "C" fizzy_status fizzy_set_fields(fizzy_ctx *c, const double *u, const do
         k_zero_plane<<<(unsigned)((c->P.sxy + 255) / 256), 256, 0, c->stream>>>(c->P, c->w);
         FZ_LAUNCHED(FZK_OTHER);
     }
-    const double init[2] = {0.0, c->P.gamma_abs};
-    FZ_CUDA(cudaMemcpyAsync(c->scal, init, sizeof(init), cudaMemcpyHostToDevice, c->stream));
-    FZ_CUDA(cudaStreamSynchronize(c->stream));  // `init` is a stack variable
+    FZ_TB(FZK_OTHER);
+    k_init_scalars<<<1, 1, 0, c->stream>>>(c->P, c->scal);   // running max|u| = 0, Gamma = gamma_abs
+    FZ_LAUNCHED(FZK_OTHER);
     FZ_TB(FZK_OTHER);
     k_absmax3<<<148 * 8, 256, 0, c->stream>>>(c->P, c->u, c->v, c->w, c->scal);
     FZ_LAUNCHED(FZK_OTHER);
@@ -474,6 +529,7 @@ extern "C" fizzy_status fizzy_get_fields(fizzy_ctx *c, double *u, double *v, dou
                                          double *T, double *p_prev)
 {
     if (!c) return FIZZY_EINVAL;
+    FZ_DEVICE();
     const size_t B = (size_t)c->N * sizeof(double);
     double *dst[] = {u, v, w, p, phi, c->heat ? T : nullptr, p_prev};
     const double *src[] = {c->u, c->v, c->w, c->p, c->phi, c->T, c->pp};
@@ -485,6 +541,7 @@ extern "C" fizzy_status fizzy_get_fields(fizzy_ctx *c, double *u, double *v, dou
 extern "C" fizzy_status fizzy_rk3_substep(fizzy_ctx *c, int stage, double dt)
 {
     if (!c) return FIZZY_EINVAL;
+    FZ_DEVICE();
     if (stage < 0 || stage > 2 || !(dt > 0.0)) return fail(c, FIZZY_EINVAL, "stage must be 0,1,2 and dt > 0");
     if (!c->fields_set) return fail(c, FIZZY_ESTATE, "fizzy_set_fields has not been called");
     if (stage != c->next_stage) return fail(c, FIZZY_ESTATE, "stages must be called in the order 0,1,2");
@@ -521,8 +578,7 @@ extern "C" fizzy_status fizzy_rk3_substep(fizzy_ctx *c, int stage, double dt)
     A.us = c->us; A.vs = c->vs; A.ws = c->ws; A.hu = c->hu; A.hv = c->hv; A.hw = c->hw;
     A.scal = c->scal; A.dt = dt; A.gs = gs; A.zs = zs; A.adt = as * dt; A.keep_h = stage != 2;
     FZ_TB(FZK_MOM);
-    if (c->varrho) { if (c->varmu) launch_momentum<true, true>(c, grid, block, A); else launch_momentum<true, false>(c, grid, block, A); }
-    else { if (c->varmu) launch_momentum<false, true>(c, grid, block, A); else launch_momentum<false, false>(c, grid, block, A); }
+    FZ_CUDA(launch_momentum(c, grid, block, &A));
     FZ_LAUNCHED(FZK_MOM);
     // S4: b = rho0/(a dt) D(u**), FFT x (fused), FFT y, tridiagonal z, inverse
     FZ_TB(FZK_FFTX_FWD);
@@ -550,6 +606,7 @@ extern "C" fizzy_status fizzy_rk3_substep(fizzy_ctx *c, int stage, double dt)
 extern "C" fizzy_status fizzy_diagnostics(fizzy_ctx *c, double *out)
 {
     if (!c) return FIZZY_EINVAL;
+    FZ_DEVICE();
     if (!out) return fail(c, FIZZY_EINVAL, "out must be non-NULL");
     if (!c->fields_set) return fail(c, FIZZY_ESTATE, "fizzy_set_fields has not been called");
     FZ_TB(FZK_OTHER);
@@ -558,7 +615,7 @@ extern "C" fizzy_status fizzy_diagnostics(fizzy_ctx *c, double *out)
     FZ_TB(FZK_OTHER);
     k_diag_final<<<1, 256, 0, c->stream>>>(c->P, c->dpart, FZ_DIAG_BLOCKS, c->scal + 8);
     FZ_LAUNCHED(FZK_OTHER);
-    FZ_CUDA(cudaMemcpyAsync(out, c->scal + 8, 6 * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    FZ_CUDA(cudaMemcpyAsync(out, c->scal + 8, 8 * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
     FZ_CUDA(cudaStreamSynchronize(c->stream));
     return FIZZY_OK;
 }
@@ -566,6 +623,7 @@ extern "C" fizzy_status fizzy_diagnostics(fizzy_ctx *c, double *out)
 extern "C" fizzy_status fizzy_poisson_solve(fizzy_ctx *c, const double *rhs, double *p)
 {
     if (!c) return FIZZY_EINVAL;
+    FZ_DEVICE();
     if (!rhs || !p) return fail(c, FIZZY_EINVAL, "rhs and p must be non-NULL");
     const FzP &P = c->P;
     const size_t B = (size_t)c->N * sizeof(double);
@@ -577,5 +635,103 @@ extern "C" fizzy_status fizzy_poisson_solve(fizzy_ctx *c, const double *rhs, dou
     fizzy_status s = run_spectral_solve(c, c->pn);
     if (s != FIZZY_OK) return s;
     FZ_CUDA(cudaMemcpyAsync(p, c->pn, B, cudaMemcpyDefault, c->stream));
+    return FIZZY_OK;
+}
+
+extern "C" fizzy_status fizzy_check_finite(fizzy_ctx *c, long long *count)
+{
+    if (!c) return FIZZY_EINVAL;
+    FZ_DEVICE();
+    if (!count) return fail(c, FIZZY_EINVAL, "count must be non-NULL");
+    unsigned long long *cnt = reinterpret_cast<unsigned long long *>(c->scal + 5);
+    FZ_CUDA(cudaMemsetAsync(cnt, 0, sizeof(*cnt), c->stream));
+    FZ_TB(FZK_OTHER);
+    k_count_nonfinite<<<148 * 8, 256, 0, c->stream>>>(c->N, c->u, c->v, c->w, c->p, c->phi, c->heat ? c->T : nullptr, cnt);
+    FZ_LAUNCHED(FZK_OTHER);
+    unsigned long long h = 0;
+    FZ_CUDA(cudaMemcpyAsync(&h, cnt, sizeof(h), cudaMemcpyDeviceToHost, c->stream));
+    FZ_CUDA(cudaStreamSynchronize(c->stream));
+    *count = (long long)h;
+    return FIZZY_OK;
+}
+
+extern "C" fizzy_status fizzy_stable_dt(fizzy_ctx *c, double cfl, double *dt)
+{
+    if (!c) return FIZZY_EINVAL;
+    FZ_DEVICE();
+    if (!dt || !(cfl > 0.0)) return fail(c, FIZZY_EINVAL, "dt must be non-NULL and cfl > 0");
+    if (!c->fields_set) return fail(c, FIZZY_ESTATE, "fizzy_set_fields has not been called");
+    const FzP &P = c->P;
+    FZ_CUDA(cudaMemsetAsync(c->scal + 3, 0, 2 * sizeof(double), c->stream));
+    FZ_TB(FZK_OTHER);
+    k_dt_reduce<<<148 * 8, 256, 0, c->stream>>>(P, c->u, c->v, c->w, c->scal + 3);
+    FZ_LAUNCHED(FZK_OTHER);
+    double red[2] = {0.0, 0.0};
+    FZ_CUDA(cudaMemcpyAsync(red, c->scal + 3, sizeof(red), cudaMemcpyDeviceToHost, c->stream));
+    FZ_CUDA(cudaStreamSynchronize(c->stream));
+    // N16: the limits are scalars of the parameters and of the two maxima just reduced on the device
+    const double S = 1.0 / (P.dx * P.dx) + 1.0 / (P.dy * P.dy) + 1.0 / (c->dzmin * c->dzmin);
+    const double dmin = std::fmin(P.dx, std::fmin(P.dy, c->dzmin));
+    const double gam = P.gamma_rel * red[1] + P.gamma_abs;
+    const double nu = std::fmax(P.mu1 / P.rho1, P.mu2 / P.rho2);
+    double lim = INFINITY;
+    if (red[0] > 0.0) lim = std::fmin(lim, 1.0 / red[0]);
+    if (nu > 0.0) lim = std::fmin(lim, 1.0 / (2.0 * nu * S));
+    if (P.sigma > 0.0) lim = std::fmin(lim, std::sqrt((P.rho1 + P.rho2) * dmin * dmin * dmin / (4.0 * M_PI * P.sigma)));
+    if (gam > 0.0) lim = std::fmin(lim, 1.0 / (2.0 * gam * P.eps * S));
+    if (P.heat) lim = std::fmin(lim, 1.0 / (2.0 * std::fmax(P.k1 / (P.rho1 * P.cp1), P.k2 / (P.rho2 * P.cp2)) * S));
+    *dt = std::isinf(lim) ? 0.0 : cfl * lim;
+    return FIZZY_OK;
+}
+
+extern "C" fizzy_status fizzy_graph_enable(fizzy_ctx *c, int on)
+{
+    if (!c) return FIZZY_EINVAL;
+    if (on && (c->stream == nullptr || c->stream == cudaStreamLegacy || c->stream == cudaStreamPerThread))
+        return fail(c, FIZZY_EINVAL, "CUDA graph capture needs a context created on a non-default stream");
+    c->graph_on = on != 0;
+    return FIZZY_OK;
+}
+
+extern "C" fizzy_status fizzy_rk3_step(fizzy_ctx *c, double dt)
+{
+    if (!c) return FIZZY_EINVAL;
+    FZ_DEVICE();
+    if (!(dt > 0.0)) return fail(c, FIZZY_EINVAL, "dt must be > 0");
+    if (!c->fields_set) return fail(c, FIZZY_ESTATE, "fizzy_set_fields has not been called");
+    if (c->next_stage != 0) return fail(c, FIZZY_ESTATE, "fizzy_rk3_step must start at stage 0");
+    fizzy_status s = FIZZY_OK;
+    if (!c->graph_on || c->timing) {   // plain launches (per-kernel events cannot be recorded into a replayed graph)
+        for (int stage = 0; stage < 3 && s == FIZZY_OK; ++stage) s = fizzy_rk3_substep(c, stage, dt);
+        return s;
+    }
+    const int par = c->phi == c->phi0 ? 0 : 1;
+    if (!c->gexec[par] || c->gdt[par] != dt || c->gkey[par][0] != c->p || c->gkey[par][1] != c->pp) {   // (re)capture: the kernel arguments bake in dt and the buffer rotation
+        if (c->gexec[par]) { cudaGraphExecDestroy(c->gexec[par]); c->gexec[par] = nullptr; }
+        // the capture itself executes nothing: remember the buffer rotation, capture, restore, then replay below
+        double *sv[] = {c->phi, c->phin, c->p, c->pp, c->pn, c->T, c->Tn};
+        const long long l0 = c->launches;
+        cudaGraph_t g = nullptr;
+        FZ_CUDA(cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeThreadLocal));
+        for (int stage = 0; stage < 3 && s == FIZZY_OK; ++stage) s = fizzy_rk3_substep(c, stage, dt);
+        const cudaError_t ce = cudaStreamEndCapture(c->stream, &g);
+        c->glaunches[par] = c->launches - l0;
+        c->launches = l0;
+        c->phi = sv[0]; c->phin = sv[1]; c->p = sv[2]; c->pp = sv[3]; c->pn = sv[4]; c->T = sv[5]; c->Tn = sv[6];
+        c->next_stage = 0;
+        if (s != FIZZY_OK) { if (g) cudaGraphDestroy(g); return s; }
+        if (ce != cudaSuccess) return cuda_fail(c, ce, "cudaStreamEndCapture");
+        const cudaError_t ie = cudaGraphInstantiate(&c->gexec[par], g, 0);
+        cudaGraphDestroy(g);
+        if (ie != cudaSuccess) { c->gexec[par] = nullptr; return cuda_fail(c, ie, "cudaGraphInstantiate"); }
+        c->gdt[par] = dt;
+        c->gkey[par][0] = c->p;
+        c->gkey[par][1] = c->pp;
+    }
+    FZ_CUDA(cudaGraphLaunch(c->gexec[par], c->stream));
+    // the host-side buffer rotation of three substeps: phi and T swap three times, the pressures rotate back
+    std::swap(c->phi, c->phin);
+    if (c->heat) std::swap(c->T, c->Tn);
+    c->launches += c->glaunches[par];
     return FIZZY_OK;
 }

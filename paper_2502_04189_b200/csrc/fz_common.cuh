@@ -14,6 +14,7 @@ struct FzP {
     long long N;               // nx*ny*nz
     long long sxy;             // nx*ny (plane stride)
     double dx, dy, idx, idy;   // spacings and reciprocals
+    double lz;                 // channel height (Nusselt number)
     // 1-D z metric tables, device pointers already offset by FZ_H (index k = -2 .. nz+1)
     const double *dzf, *dzc, *idzf, *idzc, *igz;  // igz[k] = 1/(dzc[k] + dzc[k-1])
     double rho1, rho2, mu1, mu2, k1, k2, cp1, cp2;

@@ -149,30 +149,27 @@ k_fftx_inv(FzP P, const double2 *__restrict__ spec, double *__restrict__ dst, do
 }
 
 // ---------------------------------------------------------------- host-side dispatch over log2(nx)
+// which < 0: opt the three kernels of this length in to their dynamic shared memory (once, at fizzy_create)
 template <int LOG2N>
 cudaError_t fz_fftx_launch_one(int which /*0 fwd DIV, 1 fwd plain, 2 inv*/, const FzP &P, const double *src,
                                const double *us, const double *vs, const double *ws, double coef, double2 *spec,
                                double *dst, const double2 *tw, const double *scal, cudaStream_t st)
 {
+    if (which < 0) {
+        const int sf = (int)fz_fftx_smem(LOG2N, false), si = (int)fz_fftx_smem(LOG2N, true);
+        cudaError_t e = cudaFuncSetAttribute(k_fftx_fwd<true, LOG2N>, cudaFuncAttributeMaxDynamicSharedMemorySize, sf);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_fftx_fwd<false, LOG2N>, cudaFuncAttributeMaxDynamicSharedMemorySize, sf);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_fftx_inv<LOG2N>, cudaFuncAttributeMaxDynamicSharedMemorySize, si);
+        return e;
+    }
     const int n = 1 << LOG2N;
     const int np = fx_pairs(LOG2N, which == 2);
     const size_t smem = fz_fftx_smem(LOG2N, which == 2);
     const dim3 block(n / 8, np);
     const unsigned grid = (unsigned)(((long long)P.ny * P.nz) / (2 * np));
-    cudaError_t e;
-    if (which == 0) {
-        e = cudaFuncSetAttribute(k_fftx_fwd<true, LOG2N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        k_fftx_fwd<true, LOG2N><<<grid, block, smem, st>>>(P, nullptr, us, vs, ws, coef, spec, tw);
-    } else if (which == 1) {
-        e = cudaFuncSetAttribute(k_fftx_fwd<false, LOG2N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        k_fftx_fwd<false, LOG2N><<<grid, block, smem, st>>>(P, src, nullptr, nullptr, nullptr, 1.0, spec, tw);
-    } else {
-        e = cudaFuncSetAttribute(k_fftx_inv<LOG2N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        k_fftx_inv<LOG2N><<<grid, block, smem, st>>>(P, spec, dst, coef, tw, scal);
-    }
+    if (which == 0) k_fftx_fwd<true, LOG2N><<<grid, block, smem, st>>>(P, nullptr, us, vs, ws, coef, spec, tw);
+    else if (which == 1) k_fftx_fwd<false, LOG2N><<<grid, block, smem, st>>>(P, src, nullptr, nullptr, nullptr, 1.0, spec, tw);
+    else k_fftx_inv<LOG2N><<<grid, block, smem, st>>>(P, spec, dst, coef, tw, scal);
     return cudaSuccess;
 }
 

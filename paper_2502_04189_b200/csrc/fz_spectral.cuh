@@ -247,31 +247,29 @@ k_spec_bwd(FzP P, FzTri Tt, double2 *__restrict__ spec, const double2 *__restric
 }
 
 // ---------------------------------------------------------------- host-side dispatch over log2(ny)
+// which: 0 forward sweep, 1 backward sweep, < 0: shared-memory opt-in of both kernels (once, at fizzy_create)
 template <bool CYCLIC, int LOG2N>
-cudaError_t fz_spec_launch_one(bool fwd, const FzP &P, const FzTri &Tt, double2 *spec, const double2 *tw,
+cudaError_t fz_spec_launch_one(int which, const FzP &P, const FzTri &Tt, double2 *spec, const double2 *tw,
                                double *scal, cudaStream_t st)
 {
     const int n = 1 << LOG2N;
-    const size_t smem = fz_spec_smem(n, fwd ? 0 : (CYCLIC ? 2 : 1));
-    cudaError_t e;
-    if (fwd) {
-        e = cudaFuncSetAttribute(k_spec_fwd<CYCLIC, LOG2N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        k_spec_fwd<CYCLIC, LOG2N><<<P.nxh, n / 8, smem, st>>>(P, Tt, spec, tw);
-    } else {
-        e = cudaFuncSetAttribute(k_spec_bwd<CYCLIC, LOG2N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        k_spec_bwd<CYCLIC, LOG2N><<<P.nxh, n / 8, smem, st>>>(P, Tt, spec, tw, scal);
+    const size_t sf = fz_spec_smem(n, 0), sb = fz_spec_smem(n, CYCLIC ? 2 : 1);
+    if (which < 0) {
+        cudaError_t e = cudaFuncSetAttribute(k_spec_fwd<CYCLIC, LOG2N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sf);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_spec_bwd<CYCLIC, LOG2N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sb);
+        return e;
     }
+    if (which == 0) k_spec_fwd<CYCLIC, LOG2N><<<P.nxh, n / 8, sf, st>>>(P, Tt, spec, tw);
+    else k_spec_bwd<CYCLIC, LOG2N><<<P.nxh, n / 8, sb, st>>>(P, Tt, spec, tw, scal);
     return cudaSuccess;
 }
 
 template <bool CYCLIC>
-cudaError_t fz_spec_launch(bool fwd, int log2n, const FzP &P, const FzTri &Tt, double2 *spec, const double2 *tw,
+cudaError_t fz_spec_launch(int which, int log2n, const FzP &P, const FzTri &Tt, double2 *spec, const double2 *tw,
                            double *scal, cudaStream_t st)
 {
     switch (log2n) {
-#define FZ_CASE(L_) case L_: return fz_spec_launch_one<CYCLIC, L_>(fwd, P, Tt, spec, tw, scal, st);
+#define FZ_CASE(L_) case L_: return fz_spec_launch_one<CYCLIC, L_>(which, P, Tt, spec, tw, scal, st);
         FZ_CASE(3) FZ_CASE(4) FZ_CASE(5) FZ_CASE(6) FZ_CASE(7) FZ_CASE(8) FZ_CASE(9) FZ_CASE(10)
 #undef FZ_CASE
     }

@@ -22,6 +22,13 @@ __global__ void k_absmax3(FzP P, const double *__restrict__ u, const double *__r
     if ((threadIdx.x & 31) == 0) fz_atomic_max_nonneg(umax, m);
 }
 
+// fizzy_set_fields: running max|u| = 0 (k_absmax3 follows), Gamma = gamma_abs until the first stage-0 latch
+__global__ void k_init_scalars(FzP P, double *scal)
+{
+    scal[0] = 0.0;
+    scal[1] = P.gamma_abs;
+}
+
 // scal[0] = running max|u| (reset here), scal[1] = Gamma (latched here; N15)
 __global__ void k_latch_gamma(FzP P, double *scal)
 {

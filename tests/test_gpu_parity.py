@@ -196,10 +196,84 @@ def test_diagnostics(fz, oracle_mod, name):
         o.step(dt)
         g.step(dt)
     do, dg = o.diagnostics(), g.fizzy_diagnostics()
-    for q in (0, 1, 4, 5):
+    for q in (0, 1, 4, 5, 6, 7):
         assert abs(dg[q] - do[q]) <= 1e-10 * max(abs(do[q]), 1e-300), (name, q, dg[q], do[q])
+    if cfg["heat"]:
+        assert dg[6] > 0.5 and dg[7] > 0.5      # the channel case really has a Nusselt number (conduction: 1)
     assert abs(dg[2] - do[2]) <= 1e-10 * max(do[2], 1e-300)
     umax = max(do[2], 1.0)
     assert abs(dg[3] - do[3]) <= 1e-9 * umax / min(cfg["lx"] / cfg["nx"], cfg["ly"] / cfg["ny"])
     assert np.array_equal(dg, g.fizzy_diagnostics())   # fixed-order reduction: repeatable bit for bit
+    g.close()
+
+
+@pytest.mark.parametrize("name", ["cfg1_taylor_green_64", "cfg2_bubbles_walls_64x64x48", "cfg4_channel_heat_64x32x48"])
+def test_stable_dt(fz, oracle_mod, name):
+    """fizzy_stable_dt (device reduction of the two maxima + the N16 formula) against the oracle's, on the initial
+    fields -- where it must also reproduce the dt the input recipe computed -- and after two steps."""
+    cfg, f, dt, o, g = _pair(fz, oracle_mod, name)
+    assert abs(g.fizzy_stable_dt(0.5) - dt) <= 1e-13 * dt
+    assert abs(g.fizzy_stable_dt(0.5) - o.stable_dt(0.5)) <= 1e-13 * dt
+    for _ in range(2):
+        o.step(dt)
+        g.step(dt)
+    assert abs(g.fizzy_stable_dt(0.3) - o.stable_dt(0.3)) <= 1e-9 * o.stable_dt(0.3)
+    g.close()
+
+
+@pytest.mark.parametrize("name", ["cfg0_static_drop_32", "cfg4_channel_heat_64x32x48"])
+def test_graph_replay_is_bit_identical(fz, name):
+    """fizzy_rk3_step with the three substeps captured into a CUDA graph (one per buffer rotation) must give exactly
+    the fields of the plain launches, count the same launches, survive a change of dt (re-capture), a
+    fizzy_set_fields in between and substeps issued one by one in between."""
+    import torch
+    cfg, f, dt, _ = CASES[name]()
+
+    def run(graph):
+        g = fz.Fizzy(cfg, stream=torch.cuda.Stream())
+        g.fizzy_graph_enable(graph)
+        g.set_fields_numpy(**f)
+        n0 = g.fizzy_launch_count()
+        for _ in range(5):
+            g.fizzy_rk3_step(dt)
+        for s in range(3):                       # one step through the substep call: rotates phi / T once more
+            g.fizzy_rk3_substep(s, dt)
+        for _ in range(2):
+            g.fizzy_rk3_step(0.5 * dt)           # new dt: re-capture
+        mid = g.get_fields_numpy()
+        n1 = g.fizzy_launch_count() - n0
+        g.fizzy_rk3_substep(0, dt)               # stop mid-step, reload: the pressures sit in rotated buffers now
+        g.set_fields_numpy(**{k: mid[k] for k in f})
+        g.fizzy_rk3_step(dt)
+        out = g.get_fields_numpy()
+        g.close()
+        return mid, out, n1
+
+    a_mid, a_out, na = run(False)
+    b_mid, b_out, nb = run(True)
+    assert na == nb
+    for k in a_out:
+        assert np.array_equal(a_mid[k], b_mid[k]), (name, "mid", k)
+        assert np.array_equal(a_out[k], b_out[k]), (name, "out", k)
+    g = fz.Fizzy(cfg)                            # torch's default stream is the legacy stream: no capture there
+    with pytest.raises(fz.FizzyError) as e:
+        g.fizzy_graph_enable(True)
+    assert e.value.status == fz.FIZZY_EINVAL
+    g.close()
+
+
+def test_check_finite(fz):
+    import torch
+    cfg, f, dt, _ = CASES["cfg4_channel_heat_64x32x48"]()
+    g = fz.Fizzy(cfg)
+    g.set_fields_numpy(**f)
+    g.step(dt)
+    assert g.fizzy_check_finite() == 0
+    bad = dict(f)
+    bad["T"] = f["T"].copy()
+    bad["T"][3, 4, 5] = np.nan
+    bad["u"] = f["u"].copy()
+    bad["u"][1, 1, 1] = np.inf
+    g.set_fields_numpy(**bad)
+    assert g.fizzy_check_finite() == 2
     g.close()

@@ -49,12 +49,14 @@ def algorithmic_bytes_per_cell(cfg):
     b = {
         "k_phi_update": 72.0,                                   # r phi,u,v,w,hphi,divRn  w phi,hphi,psi
         "k_iface_march": 32.0 + (24.0 if varrho else 0.0),      # r psi,phi  w kappa,divRn (+Rn x3)
-        "k_momentum": 112.0 + (40.0 if varrho else 0.0) + (8.0 if heat else 0.0),
+        # r u,v,w,phi,kappa,h x3  w u** x3, h x3 (+ r Rn x3, p_hat if rho1 != rho2; + r T with heat)
+        "k_momentum": 112.0 + (32.0 if varrho else 0.0) + (8.0 if heat else 0.0),
         "k_fftx_fwd": 24.0 + spec,
         # fused FFT_y + z-elimination: forward r spec, w spec (pivots recomputed on chip); backward r spec, INV
         # (half a complex), w spec, and E if z is periodic
         "k_spec_fwd": 2.0 * spec, "k_spec_bwd": (3.0 if not cfg["z_wall"] else 2.5) * spec,
-        "k_fftx_inv": spec + 8.0, "k_correct": 56.0,
+        "k_fftx_inv": spec + 8.0,
+        "k_correct": 56.0 + (16.0 if varrho else 0.0),          # r u** x3, p_new  w u,v,w (+ r p, w p_hat if rho1 != rho2)
     }
     if heat:
         b["k_temp_update"] = 64.0

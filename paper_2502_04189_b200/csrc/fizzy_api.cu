@@ -62,6 +62,7 @@ struct fizzy_ctx {
     double *u, *v, *w, *us, *vs, *ws, *hu, *hv, *hw;
     double *phi, *phin, *hphi;
     double *p, *pp, *pn;
+    double *phat;   // 2p - p_prev (N7), rho1 != rho2 only: written by k_correct, staged by k_momentum_march
     double *T, *Tn, *hT;
     double *kappa, *divrn, *psi, *rr, *nhx, *nhy, *nhz, *rnx, *rny, *rnz;
     double2 *spec;
@@ -124,8 +125,8 @@ size_t layout(fizzy_ctx *c, void *base, const fizzy_grid *g, const fizzy_bc *bc,
                     &x->hphi, &x->p, &x->pp, &x->pn, &x->kappa, &x->divrn, &x->psi, &x->rr, &x->nhx,
                     &x->nhy, &x->nhz};
     for (auto q : f) *q = cv.dbl(N);
-    x->rnx = x->rny = x->rnz = nullptr;
-    if (varrho) { x->rnx = cv.dbl(N); x->rny = cv.dbl(N); x->rnz = cv.dbl(N); }
+    x->rnx = x->rny = x->rnz = x->phat = nullptr;
+    if (varrho) { x->rnx = cv.dbl(N); x->rny = cv.dbl(N); x->rnz = cv.dbl(N); x->phat = cv.dbl(N); }
     x->T = x->Tn = x->hT = nullptr;
     if (pr->heat) { x->T = cv.dbl(N); x->Tn = cv.dbl(N); x->hT = cv.dbl(N); }
     x->spec = static_cast<double2 *>(cv.take(M * g->nz * sizeof(double2)));
@@ -446,7 +447,7 @@ template <bool VR, bool VM, bool HT>
 cudaError_t launch_momentum3(fizzy_ctx *c, dim3 grid, dim3 block, const FzMomArgs *Ap)
 {
     const FzP &P = c->P;
-    const size_t smem = (size_t)FzMomFields<VR, HT>::NF * MRING * MPS * sizeof(double);
+    const size_t smem = (size_t)FzMomFields<VR, HT>::NF * FzMomFields<VR, HT>::RING * MPS * sizeof(double);
     if (!Ap) return cudaFuncSetAttribute(k_momentum_march<VR, VM, HT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     const FzMomArgs &A = *Ap;
     if (P.nx >= MTX && P.ny >= MTY) {   // 2.5-D marching kernel
@@ -518,6 +519,13 @@ extern "C" fizzy_status fizzy_set_fields(fizzy_ctx *c, const double *u, const do
     FZ_TB(FZK_OTHER);
     k_absmax3<<<148 * 8, 256, 0, c->stream>>>(c->P, c->u, c->v, c->w, c->scal);
     FZ_LAUNCHED(FZK_OTHER);
+    if (c->varrho) {   // p_hat = 2p - p_prev of the loaded pressures (N7)
+        dim3 grid, block;
+        cell_launch(c, grid, block);
+        FZ_TB(FZK_OTHER);
+        k_phat<<<grid, block, 0, c->stream>>>(c->P, c->p, c->pp, c->phat);
+        FZ_LAUNCHED(FZK_OTHER);
+    }
     fizzy_status s = run_interface(c, true);
     if (s != FIZZY_OK) return s;
     c->fields_set = 1;
@@ -574,7 +582,7 @@ extern "C" fizzy_status fizzy_rk3_substep(fizzy_ctx *c, int stage, double dt)
     // S2 + S3: property map on the fly, momentum predictor -> u**
     FzMomArgs A;
     A.u = c->u; A.v = c->v; A.w = c->w; A.phi = c->phi; A.kappa = c->kappa;
-    A.rnx = c->rnx; A.rny = c->rny; A.rnz = c->rnz; A.p = c->p; A.pp = c->pp; A.T = c->T;
+    A.rnx = c->rnx; A.rny = c->rny; A.rnz = c->rnz; A.p = c->p; A.pp = c->pp; A.phat = c->phat; A.T = c->T;
     A.us = c->us; A.vs = c->vs; A.ws = c->ws; A.hu = c->hu; A.hv = c->hv; A.hw = c->hw;
     A.scal = c->scal; A.dt = dt; A.gs = gs; A.zs = zs; A.adt = as * dt; A.keep_h = stage != 2;
     FZ_TB(FZK_MOM);
@@ -587,13 +595,14 @@ extern "C" fizzy_status fizzy_rk3_substep(fizzy_ctx *c, int stage, double dt)
     FZ_LAUNCHED(FZK_FFTX_FWD);
     if ((s = run_spectral_solve(c, c->pn)) != FIZZY_OK) return s;
     // S5: correction, pressure rotation
+    // (rho1 != rho2: it also forms p_hat = 2 p_new - p for the next substep's predictor, N7)
     FZ_TB(FZK_CORRECT);
     if (stage == 2)
         k_correct<true><<<grid, block, 0, c->stream>>>(P, c->us, c->vs, c->ws, c->pn, c->u, c->v, c->w,
-                                                       as * dt / P.rho0, c->scal);
+                                                       as * dt / P.rho0, c->scal, c->p, c->phat);
     else
         k_correct<false><<<grid, block, 0, c->stream>>>(P, c->us, c->vs, c->ws, c->pn, c->u, c->v, c->w,
-                                                        as * dt / P.rho0, c->scal);
+                                                        as * dt / P.rho0, c->scal, c->p, c->phat);
     FZ_LAUNCHED(FZK_CORRECT);
     double *old_pp = c->pp;
     c->pp = c->p;

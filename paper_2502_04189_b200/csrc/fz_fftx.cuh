@@ -27,8 +27,10 @@ __host__ __device__ constexpr int fx_minb(int log2n, bool inverse) { return (!in
 // shared memory of one line pair: two padded lines + 2 elements of skew, so that the buffers of consecutive
 // pairs start 8 banks apart and the (un)tangling accesses, which touch the same l in every pair, do not collide
 #define FX_PAIR(n_) (2 * FX_LINE(n_) + 2)
-// L2 prefetch distance in CTAs: the CTAs that launch about one residency later (3-5 CTAs on each of 148 SMs)
-#define FX_AHEAD 592
+// k_fftx_inv: L2 prefetch distance in CTAs = one residency (3 CTAs on each of 148 SMs): the CTA that takes this
+// one's place finds its scattered 128-byte spectrum pieces in L2.  (The forward kernel reads whole contiguous lines
+// and gained nothing from the same prefetch at nx = 512 and lost at nx = 1024; it does not prefetch.)
+#define FX_AHEAD 444
 
 __host__ __device__ inline size_t fz_fftx_smem(int log2n, bool inverse) { return (size_t)fx_pairs(log2n, inverse) * FX_PAIR(1 << log2n) * 16; }
 
@@ -48,16 +50,6 @@ k_fftx_fwd(FzP P, const double *__restrict__ src, const double *__restrict__ us,
     const int k = (int)(L0 / P.ny), j0 = (int)(L0 - (long long)k * P.ny);
     const int ja = j0 + 2 * g;                                      // lines ja (real part), ja+1 (imaginary part)
     const long long ra = ((long long)k * P.ny + ja) * n, rb = ra + n;
-    {   // pull the input lines of the CTA FX_AHEAD launches later into L2 (one 128-byte line per thread and array):
-        // this CTA's own loads were prefetched the same way, so the load phase sees L2, not HBM, latency
-        const long long Lp = L0 + (long long)FX_AHEAD * (2 * FX_PAIRS);
-        const int tq = g * T8 + jt;                                 // 16 doubles per 128-byte line
-        if (Lp < (long long)P.ny * P.nz && tq * 16 < 2 * FX_PAIRS * n) {
-            const long long o = Lp * n + tq * 16;
-            if (DIV) { fz_prefetch_l2(us + o); fz_prefetch_l2(vs + o); fz_prefetch_l2(ws + o); }
-            else fz_prefetch_l2(src + o);
-        }
-    }
     double2 v[8];
     if (DIV) {
         const long long rm = ((long long)k * P.ny + fz_im(ja, P.ny)) * n;   // row ja-1 (periodic)

@@ -11,7 +11,7 @@
 #include "fz_common.cuh"
 
 struct FzMomArgs {
-    const double *u, *v, *w, *phi, *kappa, *rnx, *rny, *rnz, *p, *pp, *T;
+    const double *u, *v, *w, *phi, *kappa, *rnx, *rny, *rnz, *p, *pp, *phat, *T;   // phat = 2p - pp (N7), marching kernel
     double *us, *vs, *ws, *hu, *hv, *hw;
     const double *scal;  // scal[1] = Gamma
     double dt, gs, zs, adt;  // adt = (gs+zs)*dt
@@ -205,24 +205,31 @@ k_momentum(FzP P, FzMomArgs A)
 #define MPW (MTX + 4)
 #define MPH (MTY + 2)
 #define MPS (MPW * MPH)
-#define MRING 5
 #define MCHUNKS (MPS / 2)
 
+// Staged fields and ring depth.  rho1 == rho2: u, v, w, phi, kappa (+T), rings of five planes (copies issued two
+// planes ahead), three (two with heat) CTAs per SM.  rho1 != rho2: also Rn on the three faces and p_hat = 2p - p_prev
+// (formed once by k_correct, N7): nine fields, rings of FOUR planes (one plane ahead: a plane of this variant takes
+// several microseconds) = 104 KB (115 200 B with T: two CTAs of that size still fit the 228 KB of an SM), so that TWO
+// CTAs share an SM -- the variant is bound by dependent fp64 chains and needs the warps.
 template <bool VARRHO, bool HEAT>
 struct FzMomFields {
     static constexpr int U = 0, V = 1, W = 2, PHI = 3, KAP = 4;
-    static constexpr int T = 5;                        // valid if HEAT
-    static constexpr int RX = 5 + (HEAT ? 1 : 0);      // valid if VARRHO
-    static constexpr int RY = RX + 1, RZ = RX + 2, PN = RX + 3, PO = RX + 4;   // p and p_prev
-    static constexpr int NF = 5 + (HEAT ? 1 : 0) + (VARRHO ? 5 : 0);
+    static constexpr bool T_STAGED = HEAT;
+    static constexpr int T = 5;                            // valid if T_STAGED
+    static constexpr int RX = 5 + (T_STAGED ? 1 : 0);      // valid if VARRHO
+    static constexpr int RY = RX + 1, RZ = RX + 2, PH = RX + 3;
+    static constexpr int NF = 5 + (T_STAGED ? 1 : 0) + (VARRHO ? 4 : 0);
+    static constexpr int RING = VARRHO ? 4 : 5;
+    static constexpr int MINB = VARRHO ? 2 : (HEAT ? 2 : MOM_MINB);
 };
 
 template <bool VARRHO, bool VARMU, bool HEAT>
-__global__ void __launch_bounds__(MTX * MTY, (VARRHO || HEAT) ? 1 : MOM_MINB)
+__global__ void __launch_bounds__(MTX * MTY, FzMomFields<VARRHO, HEAT>::MINB)
 k_momentum_march(FzP P, FzMomArgs A, int KC)
 {
     using F = FzMomFields<VARRHO, HEAT>;
-    constexpr int NF = F::NF;
+    constexpr int NF = F::NF, MRING = F::RING;
     extern __shared__ __align__(16) double smm[];  // [NF][MRING][MPS]
     const int tx = threadIdx.x, ty = threadIdx.y, t = ty * MTX + tx;
     const int i0 = blockIdx.x * MTX, j0 = blockIdx.y * MTY;
@@ -239,11 +246,11 @@ k_momentum_march(FzP P, FzMomArgs A, int KC)
 
     const double *src[NF];
     src[F::U] = A.u; src[F::V] = A.v; src[F::W] = A.w; src[F::PHI] = A.phi; src[F::KAP] = A.kappa;
-    if (HEAT) src[F::T] = A.T;
-    if (VARRHO) { src[F::RX] = A.rnx; src[F::RY] = A.rny; src[F::RZ] = A.rnz; src[F::PN] = A.p; src[F::PO] = A.pp; }
+    if (F::T_STAGED) src[F::T] = A.T;
+    if (VARRHO) { src[F::RX] = A.rnx; src[F::RY] = A.rny; src[F::RZ] = A.rnz; src[F::PH] = A.phat; }
 
     // copy plane kk (k0-1 .. k1; ghosts: periodic wrap or wall mirror) of every field into ring slot
-    // kk mod 5.  Planes are issued in increasing order: the slot advances incrementally; offsets are
+    // kk mod MRING.  Planes are issued in increasing order: the slot advances incrementally; offsets are
     // 32-bit (fizzy_create guarantees N < 2^31).
     const unsigned sxy = (unsigned)P.sxy, ugoff = (unsigned)goff_l;
     const int zlo = P.z_wall ? 0 : P.nz - 1, zhi = P.z_wall ? P.nz - 1 : 0;   // source of plane -1 / nz
@@ -259,8 +266,8 @@ k_momentum_march(FzP P, FzMomArgs A, int KC)
         sl_is = (sl_is + 1 == MRING) ? 0 : sl_is + 1;
     };
     issue(k0 - 1); issue(k0); fz_cp_async_commit();
-    issue(k0 + 1); fz_cp_async_commit();
-    issue(k0 + 2); fz_cp_async_commit();
+#pragma unroll
+    for (int d = 1; d <= MRING - 3; ++d) { issue(k0 + d); fz_cp_async_commit(); }
 
     const double dx = P.idx, dy = P.idy;
     const double dmu = P.mu1 - P.mu2;
@@ -279,9 +286,9 @@ k_momentum_march(FzP P, FzMomArgs A, int KC)
     }
     double izc_0 = P.idzc[k0 - 1], izc_n = P.idzc[k0], izf_p = P.idzf[k0], izf_n = P.idzf[k0 + 1];
     for (int k = k0; k < k1; ++k) {
-        fz_cp_async_wait<1>();
+        fz_cp_async_wait<MRING - 4>();
         __syncthreads();
-        issue(k + 3);
+        issue(k + MRING - 2);
         fz_cp_async_commit();
         sl = (sl + 1 == MRING) ? 0 : sl + 1;
         om = o0; o0 = op; op = sl * MPS + cidx;   // planes k-1, k, k+1
@@ -331,14 +338,22 @@ k_momentum_march(FzP P, FzMomArgs A, int KC)
             irx = fz_rcp(0.5 * (r000 + P.rho2 + P.drho * fz_clip01(fp00)));
             iry = fz_rcp(0.5 * (r000 + P.rho2 + P.drho * fz_clip01(f0p0)));
             irz = fz_rcp(0.5 * (r000 + P.rho2 + P.drho * fz_clip01(f00p)));
-            // p_hat = 2 p - p_prev (N7)
-#define PH_(di, dj, o) (2.0 * S_(F::PN, di, dj, o) - S_(F::PO, di, dj, o))
-            ph000 = PH_(0, 0, o0); php00 = PH_(1, 0, o0); ph0p0 = PH_(0, 1, o0);
-            ph00p = PH_(0, 0, op);
-#undef PH_
+            // p_hat = 2 p - p_prev (N7), formed by k_correct of the previous substep
+            ph000 = S_(F::PH, 0, 0, o0); php00 = S_(F::PH, 1, 0, o0); ph0p0 = S_(F::PH, 0, 1, o0);
+            ph00p = S_(F::PH, 0, 0, op);
         }
-        double T000 = 0;
-        if (HEAT) T000 = S_(F::T, 0, 0, o0);
+        // temperature at the cell and its three "+" neighbours: staged, or straight from global memory (T_ mirrors S_)
+        double T000 = 0, Tp00 = 0, T0p0 = 0, T00p = 0;
+        if (HEAT) {
+            if (F::T_STAGED) {
+                T000 = S_(F::T, 0, 0, o0); Tp00 = S_(F::T, 1, 0, o0); T0p0 = S_(F::T, 0, 1, o0); T00p = S_(F::T, 0, 0, op);
+            } else {
+                const long long row = (long long)k * P.sxy + (long long)P.nx * j;
+                T000 = A.T[c]; Tp00 = A.T[row + fz_ip(i, P.nx)];
+                T0p0 = A.T[(long long)k * P.sxy + (long long)P.nx * fz_ip(j, P.ny) + i];
+                T00p = k < P.kzf ? A.T[c + P.sxy - (k + 1 == P.nz ? P.N : 0)] : 0.0;
+            }
+        }
         // edge viscosity (N11): mean of the four cells around the edge; a constant if mu1 == mu2
 #define MUE_(a_, b_, c_, d_) (VARMU ? 0.25 * ((a_) + (b_) + (c_) + (d_)) : P.mu2)
         // advective edge products and edge stresses on the three "+" edges of the cell, shared by
@@ -368,7 +383,7 @@ k_momentum_march(FzP P, FzMomArgs A, int KC)
                                     Rtz * (u00p - u00m) * P.igz[k]);
             }
             double B = P.gx * (1.0 - P.rho_ref * irx) + P.fx + P.a_lin * u000;
-            if (HEAT) B -= P.gx * P.beta * (0.5 * (T000 + S_(F::T, 1, 0, o0)) - P.t_ref);
+            if (HEAT) B -= P.gx * P.beta * (0.5 * (T000 + Tp00) - P.t_ref);
             const double rhs = Aa + (V + Sf + M) * irx + B;
             double un = u000 + A.dt * (A.gs * rhs + A.zs * hu_old);
             if (VARRHO) un -= A.adt * (irx - ir0) * (php00 - ph000) * dx;
@@ -396,7 +411,7 @@ k_momentum_march(FzP P, FzMomArgs A, int KC)
                                     Rtz * (v00p - v00m) * P.igz[k]);
             }
             double B = P.gy * (1.0 - P.rho_ref * iry) + P.fy + P.a_lin * v000;
-            if (HEAT) B -= P.gy * P.beta * (0.5 * (T000 + S_(F::T, 0, 1, o0)) - P.t_ref);
+            if (HEAT) B -= P.gy * P.beta * (0.5 * (T000 + T0p0) - P.t_ref);
             const double rhs = Aa + (V + Sf + M) * iry + B;
             double vn = v000 + A.dt * (A.gs * rhs + A.zs * hv_old);
             if (VARRHO) vn -= A.adt * (iry - ir0) * (ph0p0 - ph000) * dy;
@@ -427,7 +442,7 @@ k_momentum_march(FzP P, FzMomArgs A, int KC)
                                     Rtx * (wp00 - wm00) * (0.5 * dx) + Rty * (w0p0 - w0m0) * (0.5 * dy));
             }
             double B = P.gz * (1.0 - P.rho_ref * irz) + P.fz + P.a_lin * w000;
-            if (HEAT) B -= P.gz * P.beta * (0.5 * (T000 + S_(F::T, 0, 0, op)) - P.t_ref);
+            if (HEAT) B -= P.gz * P.beta * (0.5 * (T000 + T00p) - P.t_ref);
             const double rhs = Aa + (V + Sf + M) * irz + B;
             double wn = w000 + A.dt * (A.gs * rhs + A.zs * hw_old);
             if (VARRHO) wn -= A.adt * (irz - ir0) * (ph00p - ph000) * izc;

@@ -199,17 +199,20 @@ k_temp_update(FzP P, const double *__restrict__ T, const double *__restrict__ ph
 
 // ---------------------------------------------------------------- S5: velocity correction
 // u = u** - (a dt / rho0) d_a p_new  (the p_hat part of BASELINE.json:5(v) is already in u**)
+// phat != NULL (rho1 != rho2): also p_hat = 2 p_new - p_old, the extrapolated pressure of the NEXT substep (N7)
 template <bool WITH_MAX>
 __global__ void k_correct(FzP P, const double *__restrict__ us, const double *__restrict__ vs,
                           const double *__restrict__ ws, const double *__restrict__ pn,
                           double *__restrict__ u, double *__restrict__ v, double *__restrict__ w,
-                          double coef /* a dt / rho0 */, double *umax)
+                          double coef /* a dt / rho0 */, double *umax, const double *__restrict__ pold,
+                          double *__restrict__ phat)
 {
     FZ_CELL_IJK
     const FzZ z = fz_zn(P, k);
     const long long pl = (long long)P.ny * k;
     const long long c = i + P.nx * (j + pl);
     const double p0 = pn[c];
+    if (phat) phat[c] = 2.0 * p0 - pold[c];
     const double un = us[c] - coef * (pn[fz_ip(i, P.nx) + P.nx * (j + pl)] - p0) * P.idx;
     const double vn = vs[c] - coef * (pn[i + P.nx * (fz_ip(j, P.ny) + pl)] - p0) * P.idy;
     double wn = 0.0;
@@ -231,6 +234,14 @@ __global__ void k_correct(FzP P, const double *__restrict__ us, const double *__
             if (m > *reinterpret_cast<volatile double *>(umax)) fz_atomic_max_nonneg(umax, m);
         }
     }
+}
+
+// p_hat = 2p - p_prev (N7) of freshly loaded pressures
+__global__ void k_phat(FzP P, const double *__restrict__ p, const double *__restrict__ pp, double *__restrict__ phat)
+{
+    FZ_CELL_IJK
+    const long long c = i + P.nx * (j + (long long)P.ny * k);
+    phat[c] = 2.0 * p[c] - pp[c];
 }
 
 // zero the top-wall w plane (w[:,:,nz-1] == 0 with walls)

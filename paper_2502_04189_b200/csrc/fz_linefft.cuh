@@ -22,6 +22,14 @@ struct FzLineFFT {
     double2 w8[(TWREG && NP8 > 1) ? NP8 - 1 : 1][7];
     double2 wr[(TWREG && REM) ? NB : 1][REM ? R2 - 1 : 1];
     const double2 *twp;
+    // barrier between passes: the whole CTA (bar_id = 0) or only the bar_n threads (a multiple of 32) that share
+    // named barrier bar_id -- several independent line transforms can then be in flight in one CTA
+    int bar_id = 0, bar_n = 0;
+    __device__ __forceinline__ void sync() const
+    {
+        if (bar_id == 0) __syncthreads();
+        else asm volatile("bar.sync %0, %1;" ::"r"(bar_id), "r"(bar_n) : "memory");
+    }
 
     __device__ __forceinline__ double2 twv(int q) const
     {
@@ -112,11 +120,11 @@ struct FzLineFFT {
         for (int p = 0; p < NP8; ++p) {
             if (OUT_IN_REGS && p == NP8 - 1) { pass8<false, true>(p, jt, v, cur, oth); return; }
             pass8<false, false>(p, jt, v, cur, oth);
-            __syncthreads();
+            sync();
             double2 *t = cur; cur = oth; oth = t;
         }
         passr(jt, cur, oth);
-        __syncthreads();
+        sync();
 #pragma unroll
         for (int q = 0; q < 8; ++q) v[q] = oth[FZL_PADI(jt + q * T8)];
     }
@@ -128,17 +136,17 @@ struct FzLineFFT {
     {
         double2 *cur = A, *oth = B;   // pass p writes into `oth`
         pass8<true, false>(0, jt, v, cur, oth);
-        __syncthreads();
+        sync();
         { double2 *t = cur; cur = oth; oth = t; }
 #pragma unroll
         for (int p = 1; p < NP8; ++p) {
             pass8<false, false>(p, jt, v, cur, oth);
-            __syncthreads();
+            sync();
             double2 *t = cur; cur = oth; oth = t;
         }
         if (REM) {
             passr(jt, cur, oth);
-            __syncthreads();
+            sync();
             double2 *t = cur; cur = oth; oth = t;
         }
         return cur;

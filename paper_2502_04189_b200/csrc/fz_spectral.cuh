@@ -36,7 +36,6 @@ struct FzTri {
     int cyclic;
 };
 
-#define SPEC_RING 4
 // padded position of element i of a line (one double2 of padding per 8 elements)
 #define SPEC_PADI(i_) ((i_) + ((i_) >> 3))
 #define SPEC_LINE(n_) ((n_) + ((n_) >> 3))
@@ -90,51 +89,95 @@ __global__ void k_tri_tables(FzP P, FzTri Tt)
     }
 }
 
-// shared memory: scratch line | ring of SPEC_RING padded lines | `tables` rings of coefficient rows
-// (forward sweep: none; backward: INV, and E when z is periodic)
-__host__ __device__ inline size_t fz_spec_smem(int n, int tables)
+// ---------------------------------------------------------------- marching kernels, G line transforms in flight
+// One CTA per x-mode.  A plane-step is a long dependent chain (three shared-memory FFT passes, then the recurrence),
+// and there are only nxh independent x-modes, so with one transform per CTA an SM holds a warp or two and sits idle
+// most of the time.  The CTA therefore runs G groups of ny/8 threads (blockDim = (ny/8, G)): group g owns the
+// planes k = g, g+G, ...; it stages and transforms ITS plane on its own (cp.async one own-plane ahead, L2 prefetch
+// two ahead, its own named barrier inside FzLineFFT), and only the recurrence itself is serial: its state -- d', c'
+// (and the running f, h of a cyclic system), resp. x_{k+1} (and the separator X) -- lives in shared memory and is
+// handed from the group of plane k to the group of plane k+1 through a named barrier (producer bar.arrive, consumer
+// bar.sync).  Throughput per plane is then (FFT + recurrence)/G instead of their sum, until HBM binds.
+// Per group: three padded lines (current | being prefetched | scratch, rotating), backward also two rows of INV (E).
+// G = 1 (ny < 256: a group must be whole warps; ny = 1024: shared memory) degenerates to the single-transform kernel.
+// G = 4 at ny = 256, where one transform per CTA leaves an SM with less than one warp (129 CTAs of 32 threads):
+// measured 2.1x (0.209 -> 0.094 ms forward, 0.205 -> 0.100 ms backward at 256^3).  G = 1 at ny = 512: there two
+// single-transform CTAs per SM already load the shared-memory pipe to ~40-50 %, and G = 2 or 3 (with the twiddles
+// in registers, in L1 or in shared memory) measured 0.65-0.95 ms against 0.56-0.60 ms -- the handoff traffic and
+// the table reads make that pipe the limiter.  G must keep groups whole warps (ny >= 256).
+#define SPEC_FL 5    // lines per group (current | SPEC_FL-2 being prefetched by cp.async | scratch); backward: SPEC_FL-1 rows of INV (E)
+__host__ __device__ constexpr int spec_groups(int log2n) { return log2n == 8 ? 4 : 1; }
+
+__host__ __device__ inline size_t fz_spec_smem(int log2n, bool fwd, bool cyclic)
 {
-    return (size_t)SPEC_LINE(n) * 16 + (size_t)SPEC_RING * ((size_t)SPEC_LINE(n) * 16 + (size_t)n * 8 * tables);
+    const int n = 1 << log2n, nt = n / 8, G = spec_groups(log2n);
+    const size_t lines = (size_t)G * SPEC_FL * SPEC_LINE(n) * 16;
+    if (fwd) return lines + (size_t)nt * 8 * (cyclic ? 48 : 24);
+    return lines + (size_t)G * (SPEC_FL - 1) * n * 8 * (cyclic ? 2 : 1) + (size_t)nt * 8 * 16 * (cyclic ? 2 : 1) + 16;
 }
 
+__device__ __forceinline__ void fz_bar_sync(int id, int n) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(n) : "memory"); }
+__device__ __forceinline__ void fz_bar_arrive(int id, int n) { asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(n) : "memory"); }
+
 // ---------------------------------------------------------------- forward: FFT_y + elimination
-// grid = nxh CTAs (one x-mode each), block = ny/8 threads; thread jt owns the systems m = jt + q*ny/8.
-template <bool CYCLIC, int LOG2N>
-__global__ void __launch_bounds__(128)
+// thread jt of a group owns the systems m = jt + q*ny/8.  The pivots are recomputed on the fly (c' carried): the
+// forward sweep reads no table.
+template <bool CYCLIC, int LOG2N, int G>
+__global__ void __launch_bounds__(G * ((1 << LOG2N) / 8), ((1 << LOG2N) >= 512 ? 2 : 1))
 k_spec_fwd(FzP P, FzTri Tt, double2 *__restrict__ spec, const double2 *__restrict__ tw)
 {
     extern __shared__ __align__(16) double2 sms[];
     constexpr int n = 1 << LOG2N, nt = n / 8, LN = SPEC_LINE(n);
-    const int jt = threadIdx.x, nz = P.nz;
-    double2 *scratch = sms, *lines = sms + LN;
+    const int jt = threadIdx.x, g = threadIdx.y, nz = P.nz;
+    double2 *lines = sms + g * SPEC_FL * LN;
+    double2 *st_dp = sms + G * SPEC_FL * LN;                              // [q][jt]
+    double *st_cp = reinterpret_cast<double *>(st_dp + 8 * nt);
+    double2 *st_h = reinterpret_cast<double2 *>(st_cp + 8 * nt);   // cyclic only
+    double *st_f = reinterpret_cast<double *>(st_h + 8 * nt);
     FzLineFFT<LOG2N, -1> fft;
     fft.init(tw, jt);
+    if (G > 1) { fft.bar_id = 1 + G + g; fft.bar_n = nt; }
     const long long M = (long long)P.nxh * n, base = (long long)blockIdx.x * n;
-    auto issue = [&](int k) {
+    auto issue = [&](int k, int slot) {
         if (k < nz) {
-            const int slot = k & (SPEC_RING - 1);
-            const double2 *g = spec + (long long)k * M + base;
+            const double2 *gp = spec + (long long)k * M + base;
             double2 *d = lines + slot * LN;
 #pragma unroll
-            for (int q = 0; q < 8; ++q) { const int i = jt + q * nt; fz_cp_async16(d + SPEC_PADI(i), g + i); }
+            for (int q = 0; q < 8; ++q) { const int i = jt + q * nt; fz_cp_async16(d + SPEC_PADI(i), gp + i); }
         }
     };
-    for (int p = 0; p < SPEC_RING - 1; ++p) { issue(p); fz_cp_async_commit(); }
-    double2 dp[8], h[8], v[8];
-    double f[8], lam[8], cp[8];   // the pivots are recomputed on the fly (c' carried): the forward sweep reads no table
+#pragma unroll
+    for (int d = 0; d < SPEC_FL - 2; ++d) { issue(g + d * G, d); fz_cp_async_commit(); }
+    double lam[8];
     const double c_last = Tt.c[nz - 1], a_last = Tt.a[nz - 1];
     const double lamx = Tt.lamx[blockIdx.x];
 #pragma unroll
-    for (int q = 0; q < 8; ++q) {
-        dp[q] = make_double2(0, 0); h[q] = make_double2(0, 0); f[q] = c_last;
-        lam[q] = lamx + Tt.lamy[jt + q * nt]; cp[q] = 0.0;
-    }
-    for (int k = 0; k < nz; ++k) {
-        fz_cp_async_wait<SPEC_RING - 2>();
-        __syncthreads();
-        issue(k + SPEC_RING - 1);
+    for (int q = 0; q < 8; ++q) lam[q] = lamx + Tt.lamy[jt + q * nt];
+    double2 dp[8], h[8];
+    double f[8], cp[8];
+    int cur = 0;
+    for (int k = g; k < nz; k += G) {
+        // slots: cur | cur+1 .. cur+SPEC_FL-3 in flight | cur+SPEC_FL-2 = the one issued now | cur-1 = scratch
+        const int nxt = cur + 1 == SPEC_FL ? 0 : cur + 1, scr = cur == 0 ? SPEC_FL - 1 : cur - 1;
+        const int tgt = cur + SPEC_FL - 2 >= SPEC_FL ? cur - 2 : cur + SPEC_FL - 2;
+        fz_cp_async_wait<SPEC_FL - 3>();
+        fft.sync();
+        issue(k + (SPEC_FL - 2) * G, tgt);
         fz_cp_async_commit();
-        fft.smem_to_regs(jt, lines + (k & (SPEC_RING - 1)) * LN, scratch, v);
+        double2 v[8];
+        fft.smem_to_regs(jt, lines + cur * LN, lines + scr * LN, v);
+        // the recurrence state of plane k-1 (token from its group)
+        if (k == 0) {
+#pragma unroll
+            for (int q = 0; q < 8; ++q) { dp[q] = make_double2(0, 0); h[q] = make_double2(0, 0); f[q] = c_last; cp[q] = 0.0; }
+        } else if (G > 1) {
+            fz_bar_sync(1 + g, 2 * nt);
+#pragma unroll
+            for (int q = 0; q < 8; ++q) {
+                dp[q] = st_dp[q * nt + jt]; cp[q] = st_cp[q * nt + jt];
+                if (CYCLIC) { h[q] = st_h[q * nt + jt]; f[q] = st_f[q * nt + jt]; }
+            }
+        }
         double2 *out = spec + (long long)k * M + base;
         const double a = Tt.a[k], cfull = Tt.c[k];
         if (!CYCLIC || k < nz - 1) {
@@ -144,7 +187,6 @@ k_spec_fwd(FzP P, FzTri Tt, double2 *__restrict__ spec, const double2 *__restric
             const bool sing = !CYCLIC && k == nz - 1 && blockIdx.x == 0 && jt == 0;
 #pragma unroll
             for (int q = 0; q < 8; ++q) {
-                const int m = jt + q * nt;
                 double inv = fz_rcp_signed(fz_tri_den(a, cfull, lam[q], cp[q]));
                 if (q == 0 && sing) inv = 0.0;
                 cp[q] = ck * inv;
@@ -156,8 +198,17 @@ k_spec_fwd(FzP P, FzTri Tt, double2 *__restrict__ spec, const double2 *__restric
                     h[q].y += fk * dp[q].y;
                     f[q] = -fk * (ck * inv);
                 }
-                out[m] = dp[q];
             }
+            if (G > 1 && k < nz - 1) {   // hand the state to the group of plane k+1
+#pragma unroll
+                for (int q = 0; q < 8; ++q) {
+                    st_dp[q * nt + jt] = dp[q]; st_cp[q * nt + jt] = cp[q];
+                    if (CYCLIC) { st_h[q * nt + jt] = h[q]; st_f[q * nt + jt] = f[q]; }
+                }
+                fz_bar_arrive(1 + (g + 1 == G ? 0 : g + 1), 2 * nt);
+            }
+#pragma unroll
+            for (int q = 0; q < 8; ++q) out[jt + q * nt] = dp[q];
         } else {   // last row of a cyclic system: the separator X
 #pragma unroll
             for (int q = 0; q < 8; ++q) {
@@ -166,58 +217,80 @@ k_spec_fwd(FzP P, FzTri Tt, double2 *__restrict__ spec, const double2 *__restric
                 out[m] = make_double2((v[q].x - h[q].x) * gi, (v[q].y - h[q].y) * gi);
             }
         }
+        cur = nxt;
     }
     fz_cp_async_wait<0>();
 }
 
 // ---------------------------------------------------------------- backward: substitution + inverse FFT_y
-// k descends from nz-1 to 0.  scal[2] receives the dzf-weighted mean of mode (0,0) (gauge, N17).
-template <bool CYCLIC, int LOG2N>
-__global__ void __launch_bounds__(128)
+// k descends from nz-1 to 0 (step s = nz-1-k; group g owns the steps s = g, g+G, ...).  scal[2] receives the
+// dzf-weighted mean of mode (0,0) (gauge, N17), accumulated in plane order under the token.
+template <bool CYCLIC, int LOG2N, int G>
+__global__ void __launch_bounds__(G * ((1 << LOG2N) / 8), ((1 << LOG2N) >= 512 ? 2 : 1))
 k_spec_bwd(FzP P, FzTri Tt, double2 *__restrict__ spec, const double2 *__restrict__ tw,
            double *__restrict__ scal)
 {
     extern __shared__ __align__(16) double2 sms[];
-    constexpr int n = 1 << LOG2N, nt = n / 8, LN = SPEC_LINE(n);
-    const int jt = threadIdx.x, nz = P.nz;
-    double2 *scratch = sms, *lines = sms + LN;
-    double *invs = reinterpret_cast<double *>(lines + SPEC_RING * LN);
-    double *es = invs + SPEC_RING * n;   // cyclic only
+    constexpr int n = 1 << LOG2N, nt = n / 8, LN = SPEC_LINE(n), NT = CYCLIC ? 2 : 1;
+    const int jt = threadIdx.x, g = threadIdx.y, nz = P.nz;
+    constexpr int RR = SPEC_FL - 1;                                 // ring of coefficient rows: current + in flight
+    double2 *lines = sms + g * SPEC_FL * LN;
+    double *rows0 = reinterpret_cast<double *>(sms + G * SPEC_FL * LN);
+    double *rows = rows0 + g * RR * n * NT;                         // [slot][INV | E][n]
+    double2 *st_x = reinterpret_cast<double2 *>(rows0 + G * RR * n * NT);   // [q][jt]
+    double2 *st_X = st_x + 8 * nt;                                  // cyclic only
+    double *st_acc = reinterpret_cast<double *>(st_x + 8 * nt * NT);
     FzLineFFT<LOG2N, +1> fft;
     fft.init(tw, jt);
+    if (G > 1) { fft.bar_id = 1 + G + g; fft.bar_n = nt; }
     const long long M = (long long)P.nxh * n, base = (long long)blockIdx.x * n;
-    auto issue = [&](int s) {   // step s handles plane k = nz-1-s
+    auto issue = [&](int s, int slot, int rslot) {   // step s handles plane k = nz-1-s
         if (s < nz) {
-            const int slot = s & (SPEC_RING - 1), k = nz - 1 - s;
-            const double2 *g = spec + (long long)k * M + base;
+            const int k = nz - 1 - s;
+            const double2 *gp = spec + (long long)k * M + base;
             double2 *d = lines + slot * LN;
 #pragma unroll
-            for (int q = 0; q < 8; ++q) { const int i = jt + q * nt; fz_cp_async16(d + SPEC_PADI(i), g + i); }
+            for (int q = 0; q < 8; ++q) { const int i = jt + q * nt; fz_cp_async16(d + SPEC_PADI(i), gp + i); }
             const double *gi = Tt.inv + (long long)k * M + base;
             const double *ge = Tt.e + (long long)k * M + base;
+            double *dr = rows + rslot * n * NT;
 #pragma unroll
             for (int q = 0; q < 4; ++q) {
                 const int i = 2 * (jt + q * nt);
-                fz_cp_async16(invs + slot * n + i, gi + i);
-                if (CYCLIC) fz_cp_async16(es + slot * n + i, ge + i);
+                fz_cp_async16(dr + i, gi + i);
+                if (CYCLIC) fz_cp_async16(dr + n + i, ge + i);
             }
         }
     };
-    for (int p = 0; p < SPEC_RING - 1; ++p) { issue(p); fz_cp_async_commit(); }
+#pragma unroll
+    for (int d = 0; d < SPEC_FL - 2; ++d) { issue(g + d * G, d, d); fz_cp_async_commit(); }
     double2 xn[8], X[8];
 #pragma unroll
     for (int q = 0; q < 8; ++q) { xn[q] = make_double2(0, 0); X[q] = make_double2(0, 0); }
     const int nrow = CYCLIC ? nz - 1 : nz;
     const bool gauge = blockIdx.x == 0 && jt == 0;   // owner of mode (l, m) = (0, 0)
-    double acc = 0.0, vol = 0.0;
-    for (int s = 0; s < nz; ++s) {
+    int cur = 0, rcur = 0;
+    bool first = true;
+    for (int s = g; s < nz; s += G) {
         const int k = nz - 1 - s;
-        fz_cp_async_wait<SPEC_RING - 2>();
-        __syncthreads();
-        issue(s + SPEC_RING - 1);
+        const int nxt = cur + 1 == SPEC_FL ? 0 : cur + 1, scr = cur == 0 ? SPEC_FL - 1 : cur - 1;
+        const int tgt = cur + SPEC_FL - 2 >= SPEC_FL ? cur - 2 : cur + SPEC_FL - 2;
+        const int rtgt = rcur + RR - 1 >= RR ? rcur - 1 : rcur + RR - 1;
+        fz_cp_async_wait<SPEC_FL - 3>();
+        fft.sync();
+        issue(s + (SPEC_FL - 2) * G, tgt, rtgt);
         fz_cp_async_commit();
-        double2 *ln = lines + (s & (SPEC_RING - 1)) * LN;
-        const double *iv = invs + (s & (SPEC_RING - 1)) * n, *ev = es + (s & (SPEC_RING - 1)) * n;
+        double2 *ln = lines + cur * LN;
+        const double *iv = rows + rcur * n * NT, *ev = iv + n;
+        if (G > 1 && s > 0) {   // x_{k+1} (and, once, the separator) from the group of plane k+1
+            fz_bar_sync(1 + g, 2 * nt);
+#pragma unroll
+            for (int q = 0; q < 8; ++q) {
+                xn[q] = st_x[q * nt + jt];
+                if (CYCLIC && first) X[q] = st_X[q * nt + jt];
+            }
+        }
+        first = false;
         const double ck = (k == nrow - 1) ? 0.0 : Tt.c[k];
 #pragma unroll
         for (int q = 0; q < 8; ++q) {
@@ -233,16 +306,31 @@ k_spec_bwd(FzP P, FzTri Tt, double2 *__restrict__ spec, const double2 *__restric
             }
             xn[q] = x;
         }
-        if (gauge) { acc += xn[0].x * P.dzf[k]; vol += P.dzf[k]; }
+        if (gauge) {
+            double acc = s == 0 ? 0.0 : st_acc[0], vol = s == 0 ? 0.0 : st_acc[1];
+            acc += xn[0].x * P.dzf[k];
+            vol += P.dzf[k];
+            st_acc[0] = acc; st_acc[1] = vol;
+            if (s == nz - 1) scal[2] = acc / vol;
+        }
+        if (G > 1 && s < nz - 1) {
+#pragma unroll
+            for (int q = 0; q < 8; ++q) {
+                st_x[q * nt + jt] = xn[q];
+                if (CYCLIC && s == 0) st_X[q * nt + jt] = X[q];
+            }
+            fz_bar_arrive(1 + (g + 1 == G ? 0 : g + 1), 2 * nt);
+        }
         double2 v[8];
 #pragma unroll
         for (int q = 0; q < 8; ++q) v[q] = xn[q];
-        const double2 *res = fft.regs_to_smem(jt, ln, scratch, v);
+        const double2 *res = fft.regs_to_smem(jt, ln, lines + scr * LN, v);
         double2 *out = spec + (long long)k * M + base;
 #pragma unroll
         for (int q = 0; q < 8; ++q) { const int m = jt + q * nt; out[m] = res[SPEC_PADI(m)]; }
+        cur = nxt;
+        rcur = rcur + 1 == RR ? 0 : rcur + 1;
     }
-    if (gauge) scal[2] = acc / vol;
     fz_cp_async_wait<0>();
 }
 
@@ -252,15 +340,15 @@ template <bool CYCLIC, int LOG2N>
 cudaError_t fz_spec_launch_one(int which, const FzP &P, const FzTri &Tt, double2 *spec, const double2 *tw,
                                double *scal, cudaStream_t st)
 {
-    const int n = 1 << LOG2N;
-    const size_t sf = fz_spec_smem(n, 0), sb = fz_spec_smem(n, CYCLIC ? 2 : 1);
+    constexpr int n = 1 << LOG2N, GF = spec_groups(LOG2N), GB = spec_groups(LOG2N);
+    const size_t sf = fz_spec_smem(LOG2N, true, CYCLIC), sb = fz_spec_smem(LOG2N, false, CYCLIC);
     if (which < 0) {
-        cudaError_t e = cudaFuncSetAttribute(k_spec_fwd<CYCLIC, LOG2N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sf);
-        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_spec_bwd<CYCLIC, LOG2N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sb);
+        cudaError_t e = cudaFuncSetAttribute(k_spec_fwd<CYCLIC, LOG2N, GF>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sf);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_spec_bwd<CYCLIC, LOG2N, GB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sb);
         return e;
     }
-    if (which == 0) k_spec_fwd<CYCLIC, LOG2N><<<P.nxh, n / 8, sf, st>>>(P, Tt, spec, tw);
-    else k_spec_bwd<CYCLIC, LOG2N><<<P.nxh, n / 8, sb, st>>>(P, Tt, spec, tw, scal);
+    if (which == 0) k_spec_fwd<CYCLIC, LOG2N, GF><<<P.nxh, dim3(n / 8, GF), sf, st>>>(P, Tt, spec, tw);
+    else k_spec_bwd<CYCLIC, LOG2N, GB><<<P.nxh, dim3(n / 8, GB), sb, st>>>(P, Tt, spec, tw, scal);
     return cudaSuccess;
 }
 

@@ -79,8 +79,16 @@ struct FzLineFFT {
         }
         if (p > 0) {
             const int Nsp = 1 << (3 * p), kt = (jt & (Nsp - 1)) * (N / (Nsp * 8));
+            if (TWREG) {
 #pragma unroll
-            for (int r = 1; r < 8; ++r) v[r] = fz_cmul(v[r], TWREG ? w8[p - 1][r - 1] : twv(r * kt));
+                for (int r = 1; r < 8; ++r) v[r] = fz_cmul(v[r], w8[p - 1][r - 1]);
+            } else {
+                // ONE table read per pass; w^2 .. w^7 by six complex products (depth 3, a few ulp): seven scattered
+                // 16-byte reads per pass made the L1 data pipe the limiter of the x transforms (ncu r2a: 94 %)
+                const double2 w1 = twv(kt), w2 = fz_cmul(w1, w1), w3 = fz_cmul(w2, w1), w4 = fz_cmul(w2, w2);
+                v[1] = fz_cmul(v[1], w1); v[2] = fz_cmul(v[2], w2); v[3] = fz_cmul(v[3], w3); v[4] = fz_cmul(v[4], w4);
+                v[5] = fz_cmul(v[5], fz_cmul(w4, w1)); v[6] = fz_cmul(v[6], fz_cmul(w4, w2)); v[7] = fz_cmul(v[7], fz_cmul(w4, w3));
+            }
         }
         fz_dft8<SGN>(v);
         if (!OUT_REG) {

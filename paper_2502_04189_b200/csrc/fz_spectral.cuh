@@ -105,15 +105,17 @@ __global__ void k_tri_tables(FzP P, FzTri Tt)
 // single-transform CTAs per SM already load the shared-memory pipe to ~40-50 %, and G = 2 or 3 (with the twiddles
 // in registers, in L1 or in shared memory) measured 0.65-0.95 ms against 0.56-0.60 ms -- the handoff traffic and
 // the table reads make that pipe the limiter.  G must keep groups whole warps (ny >= 256).
-#define SPEC_FL 5    // lines per group (current | SPEC_FL-2 being prefetched by cp.async | scratch); backward: SPEC_FL-1 rows of INV (E)
+#define SPEC_FL 5    // lines per group: one fixed scratch line + a ring of SPEC_FL-1 (current | SPEC_FL-2 being prefetched by
+                     // cp.async); backward: also SPEC_FL-1 rows of INV (E)
 __host__ __device__ constexpr int spec_groups(int log2n) { return log2n == 8 ? 4 : 1; }
 
 __host__ __device__ inline size_t fz_spec_smem(int log2n, bool fwd, bool cyclic)
 {
     const int n = 1 << log2n, nt = n / 8, G = spec_groups(log2n);
     const size_t lines = (size_t)G * SPEC_FL * SPEC_LINE(n) * 16;
-    if (fwd) return lines + (size_t)nt * 8 * (cyclic ? 48 : 24);
-    return lines + (size_t)G * (SPEC_FL - 1) * n * 8 * (cyclic ? 2 : 1) + (size_t)nt * 8 * 16 * (cyclic ? 2 : 1) + 16;
+    const size_t state = G > 1 ? 1 : 0;   // the handoff buffers exist only when there is somebody to hand over to
+    if (fwd) return lines + state * nt * 8 * (cyclic ? 48 : 24);
+    return lines + (size_t)G * (SPEC_FL - 1) * n * 8 * (cyclic ? 2 : 1) + state * nt * 8 * 16 * (cyclic ? 2 : 1) + 16;
 }
 
 __device__ __forceinline__ void fz_bar_sync(int id, int n) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(n) : "memory"); }
@@ -129,7 +131,7 @@ k_spec_fwd(FzP P, FzTri Tt, double2 *__restrict__ spec, const double2 *__restric
     extern __shared__ __align__(16) double2 sms[];
     constexpr int n = 1 << LOG2N, nt = n / 8, LN = SPEC_LINE(n);
     const int jt = threadIdx.x, g = threadIdx.y, nz = P.nz;
-    double2 *lines = sms + g * SPEC_FL * LN;
+    double2 *scratch = sms + g * SPEC_FL * LN, *lines = scratch + LN;   // ring of RL = SPEC_FL-1 lines
     double2 *st_dp = sms + G * SPEC_FL * LN;                              // [q][jt]
     double *st_cp = reinterpret_cast<double *>(st_dp + 8 * nt);
     double2 *st_h = reinterpret_cast<double2 *>(st_cp + 8 * nt);   // cyclic only
@@ -157,15 +159,15 @@ k_spec_fwd(FzP P, FzTri Tt, double2 *__restrict__ spec, const double2 *__restric
     double f[8], cp[8];
     int cur = 0;
     for (int k = g; k < nz; k += G) {
-        // slots: cur | cur+1 .. cur+SPEC_FL-3 in flight | cur+SPEC_FL-2 = the one issued now | cur-1 = scratch
-        const int nxt = cur + 1 == SPEC_FL ? 0 : cur + 1, scr = cur == 0 ? SPEC_FL - 1 : cur - 1;
-        const int tgt = cur + SPEC_FL - 2 >= SPEC_FL ? cur - 2 : cur + SPEC_FL - 2;
+        // ring slots: cur | cur+1 .. cur+RL-2 in flight | cur-1 = the slot the previous plane left, issued now
+        constexpr int RL = SPEC_FL - 1;
+        const int nxt = cur + 1 == RL ? 0 : cur + 1, tgt = cur == 0 ? RL - 1 : cur - 1;
         fz_cp_async_wait<SPEC_FL - 3>();
         fft.sync();
         issue(k + (SPEC_FL - 2) * G, tgt);
         fz_cp_async_commit();
         double2 v[8];
-        fft.smem_to_regs(jt, lines + cur * LN, lines + scr * LN, v);
+        fft.smem_to_regs(jt, lines + cur * LN, scratch, v);
         // the recurrence state of plane k-1 (token from its group)
         if (k == 0) {
 #pragma unroll
@@ -234,12 +236,12 @@ k_spec_bwd(FzP P, FzTri Tt, double2 *__restrict__ spec, const double2 *__restric
     constexpr int n = 1 << LOG2N, nt = n / 8, LN = SPEC_LINE(n), NT = CYCLIC ? 2 : 1;
     const int jt = threadIdx.x, g = threadIdx.y, nz = P.nz;
     constexpr int RR = SPEC_FL - 1;                                 // ring of coefficient rows: current + in flight
-    double2 *lines = sms + g * SPEC_FL * LN;
+    double2 *scratch = sms + g * SPEC_FL * LN, *lines = scratch + LN;   // ring of RR lines
     double *rows0 = reinterpret_cast<double *>(sms + G * SPEC_FL * LN);
     double *rows = rows0 + g * RR * n * NT;                         // [slot][INV | E][n]
     double2 *st_x = reinterpret_cast<double2 *>(rows0 + G * RR * n * NT);   // [q][jt]
     double2 *st_X = st_x + 8 * nt;                                  // cyclic only
-    double *st_acc = reinterpret_cast<double *>(st_x + 8 * nt * NT);
+    double *st_acc = reinterpret_cast<double *>(st_x + (G > 1 ? 8 * nt * NT : 0));   // G = 1: no handoff buffers
     FzLineFFT<LOG2N, +1> fft;
     fft.init(tw, jt);
     if (G > 1) { fft.bar_id = 1 + G + g; fft.bar_n = nt; }
@@ -269,19 +271,17 @@ k_spec_bwd(FzP P, FzTri Tt, double2 *__restrict__ spec, const double2 *__restric
     for (int q = 0; q < 8; ++q) { xn[q] = make_double2(0, 0); X[q] = make_double2(0, 0); }
     const int nrow = CYCLIC ? nz - 1 : nz;
     const bool gauge = blockIdx.x == 0 && jt == 0;   // owner of mode (l, m) = (0, 0)
-    int cur = 0, rcur = 0;
+    int cur = 0;
     bool first = true;
     for (int s = g; s < nz; s += G) {
         const int k = nz - 1 - s;
-        const int nxt = cur + 1 == SPEC_FL ? 0 : cur + 1, scr = cur == 0 ? SPEC_FL - 1 : cur - 1;
-        const int tgt = cur + SPEC_FL - 2 >= SPEC_FL ? cur - 2 : cur + SPEC_FL - 2;
-        const int rtgt = rcur + RR - 1 >= RR ? rcur - 1 : rcur + RR - 1;
+        const int nxt = cur + 1 == RR ? 0 : cur + 1, tgt = cur == 0 ? RR - 1 : cur - 1;   // lines and rows rotate together
         fz_cp_async_wait<SPEC_FL - 3>();
         fft.sync();
-        issue(s + (SPEC_FL - 2) * G, tgt, rtgt);
+        issue(s + (SPEC_FL - 2) * G, tgt, tgt);
         fz_cp_async_commit();
         double2 *ln = lines + cur * LN;
-        const double *iv = rows + rcur * n * NT, *ev = iv + n;
+        const double *iv = rows + cur * n * NT, *ev = iv + n;
         if (G > 1 && s > 0) {   // x_{k+1} (and, once, the separator) from the group of plane k+1
             fz_bar_sync(1 + g, 2 * nt);
 #pragma unroll
@@ -324,12 +324,11 @@ k_spec_bwd(FzP P, FzTri Tt, double2 *__restrict__ spec, const double2 *__restric
         double2 v[8];
 #pragma unroll
         for (int q = 0; q < 8; ++q) v[q] = xn[q];
-        const double2 *res = fft.regs_to_smem(jt, ln, lines + scr * LN, v);
+        const double2 *res = fft.regs_to_smem(jt, ln, scratch, v);
         double2 *out = spec + (long long)k * M + base;
 #pragma unroll
         for (int q = 0; q < 8; ++q) { const int m = jt + q * nt; out[m] = res[SPEC_PADI(m)]; }
         cur = nxt;
-        rcur = rcur + 1 == RR ? 0 : rcur + 1;
     }
     fz_cp_async_wait<0>();
 }

@@ -67,7 +67,7 @@ struct fizzy_ctx {
     double *kappa, *divrn, *psi, *rr, *nhx, *nhy, *nhz, *rnx, *rny, *rnz;
     double2 *spec;
     double2 *twx, *twy;
-    double *scal;  // [0] running max|u|, [1] Gamma, [2] gauge mean, [3..4] dt maxima, [5] non-finite count, [8..15] diagnostics
+    double *scal;  // [0] running max|u|, [1] Gamma, [2], [6] gauge mean (two parts), [3..4] dt maxima, [5] non-finite count, [8..15] diagnostics
     double dzmin;  // smallest cell height (N16)
     // one RK3 step as a CUDA graph (fizzy_graph_enable): one executable graph per parity of the step counter,
     // because phi/phi_new (and T/T_new) swap three times per step and are back in place after two steps
@@ -131,8 +131,10 @@ size_t layout(fizzy_ctx *c, void *base, const fizzy_grid *g, const fizzy_bc *bc,
     if (pr->heat) { x->T = cv.dbl(N); x->Tn = cv.dbl(N); x->hT = cv.dbl(N); }
     x->spec = static_cast<double2 *>(cv.take(M * g->nz * sizeof(double2)));
     x->tri.inv = cv.dbl(M * g->nz);
-    x->tri.e = x->tri.ginv = nullptr;
-    if (cyclic) { x->tri.e = cv.dbl(M * g->nz); x->tri.ginv = cv.dbl(M); }
+    x->tri.e = nullptr;
+    if (cyclic) x->tri.e = cv.dbl(M * g->nz);
+    x->tri.mid = cv.dbl(M * (cyclic ? 4 : 1));
+    x->tri.side = static_cast<double2 *>(cv.take(4 * M * sizeof(double2)));
     for (int q = 0; q < 5; ++q) { double *t = cv.dbl(g->nz + 2 * FZ_H); if (ztab) ztab[q] = t; }
     for (int q = 0; q < 2; ++q) { double *t = cv.dbl(g->nz); if (acoef) acoef[q] = t; }
     { double *t = cv.dbl(nxh); if (lam) lam[0] = t; t = cv.dbl(g->ny); if (lam) lam[1] = t; }

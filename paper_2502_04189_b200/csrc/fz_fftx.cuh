@@ -88,7 +88,7 @@ k_fftx_fwd(FzP P, const double *__restrict__ src, const double *__restrict__ us,
 }
 
 // ---------------------------------------------------------------- FFT along x, backward (c2r)
-// out = Re / Im of the inverse transform * scale - gauge shift (N17: scal[2] = mean of mode (0,0),
+// out = Re / Im of the inverse transform * scale - gauge shift (N17: scal[2] + scal[6] = mean of mode (0,0),
 // written by k_spec_bwd)
 template <int LOG2N>
 __global__ void __launch_bounds__(fx_pairs(LOG2N, true) * ((1 << LOG2N) / 8), fx_minb(LOG2N, true))
@@ -103,7 +103,7 @@ k_fftx_inv(FzP P, const double2 *__restrict__ spec, double *__restrict__ dst, do
     fft.init(tw, jt);
     const long long L0 = (long long)blockIdx.x * (2 * FX_PAIRS);
     const int k = (int)(L0 / P.ny), j0 = (int)(L0 - (long long)k * P.ny);
-    const double shift = scal[2] * scale;
+    const double shift = (scal[2] + scal[6]) * scale;
     const int nth = T8 * FX_PAIRS, t = g * T8 + jt;
     const int nxh = P.nxh;
     const double2 *in = spec + (long long)k * nxh * P.ny + j0;

@@ -48,6 +48,9 @@ def algorithmic_bytes_per_cell(cfg):
     heat = bool(cfg["heat"])
     b = {
         "k_phi_update": 72.0,                                   # r phi,u,v,w,hphi,divRn  w phi,hphi,psi
+        # S5 of the previous substep fused in front of S1 (stages 1, 2): r u** x3, p_new, phi, hphi, divRn  w u,v,w, phi, hphi, psi
+        # (+ r p_old, w p_hat if rho1 != rho2)
+        "k_corr_phi": 104.0 + (16.0 if varrho else 0.0),
         "k_iface_march": 32.0 + (24.0 if varrho else 0.0),      # r psi,phi  w kappa,divRn (+Rn x3)
         # r u,v,w,phi,kappa,h x3  w u** x3, h x3 (+ r Rn x3, p_hat if rho1 != rho2; + r T with heat)
         "k_momentum": 112.0 + (32.0 if varrho else 0.0) + (8.0 if heat else 0.0),

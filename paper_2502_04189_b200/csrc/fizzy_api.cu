@@ -37,10 +37,10 @@ struct Carver {  // hands out 256-byte aligned pieces of the workspace (or just 
 
 }  // namespace
 
-enum FzKernelId { FZK_LATCH, FZK_PHI, FZK_IMARCH, FZK_IPSI, FZK_INHAT, FZK_IFLUX, FZK_TEMP, FZK_MOM, FZK_FFTX_FWD,
+enum FzKernelId { FZK_LATCH, FZK_PHI, FZK_CORRPHI, FZK_IMARCH, FZK_IPSI, FZK_INHAT, FZK_IFLUX, FZK_TEMP, FZK_MOM, FZK_FFTX_FWD,
                   FZK_SPEC_FWD, FZK_SPEC_BWD, FZK_FFTX_INV, FZK_CORRECT, FZK_OTHER, FZK_COUNT };
 static const char *const FZK_NAME[FZK_COUNT] = {
-    "k_latch_gamma", "k_phi_update", "k_iface_march", "k_iface_psi", "k_iface_nhat", "k_iface_flux", "k_temp_update", "k_momentum",
+    "k_latch_gamma", "k_phi_update", "k_corr_phi", "k_iface_march", "k_iface_psi", "k_iface_nhat", "k_iface_flux", "k_temp_update", "k_momentum",
     "k_fftx_fwd", "k_spec_fwd", "k_spec_bwd", "k_fftx_inv", "k_correct", "other"};
 
 struct FzTimed { int id; cudaEvent_t e0, e1; };
@@ -80,6 +80,10 @@ struct fizzy_ctx {
     double *dpart; // block partials of k_diag
     FzTri tri;
     int fields_set, next_stage;
+    // S5 of stages 0 and 1 is deferred into the first kernel of the next substep (k_corr_phi): until then u, v, w
+    // still hold the velocity of the stage start and corr_coef = a dt / rho0 of the pending correction
+    bool corr_pending = false;
+    double corr_coef = 0.0;
     long long launches;
     std::string err;
 };
@@ -478,6 +482,27 @@ cudaError_t launch_momentum(fizzy_ctx *c, dim3 grid, dim3 block, const FzMomArgs
     return c->varmu ? launch_momentum2<false, true>(c, grid, block, A) : launch_momentum2<false, false>(c, grid, block, A);
 }
 
+// a deferred S5 (see corr_pending): form u, v, w now.  Every entry point that reads or replaces the velocity outside
+// a substep calls this first, so the deferral is invisible through the ABI.
+fizzy_status flush_correct(fizzy_ctx *c)
+{
+    if (!c->corr_pending) return FIZZY_OK;
+    dim3 grid, block;
+    cell_launch(c, grid, block);
+    FZ_TB(FZK_CORRECT);
+    // the pressures have rotated already: c->p is p_new, c->pp the pressure before it
+    k_correct<false><<<grid, block, 0, c->stream>>>(c->P, c->us, c->vs, c->ws, c->p, c->u, c->v, c->w, c->corr_coef,
+                                                    c->scal, c->pp, c->phat);
+    FZ_LAUNCHED(FZK_CORRECT);
+    c->corr_pending = false;
+    return FIZZY_OK;
+}
+#define FZ_FLUSH()                                       \
+    do {                                                 \
+        const fizzy_status fs_ = flush_correct(c);       \
+        if (fs_ != FIZZY_OK) return fs_;                 \
+    } while (0)
+
 // every entry point after fizzy_create: the context's device must be the current one
 fizzy_status check_device(fizzy_ctx *c)
 {
@@ -500,6 +525,7 @@ extern "C" fizzy_status fizzy_set_fields(fizzy_ctx *c, const double *u, const do
 {
     if (!c) return FIZZY_EINVAL;
     FZ_DEVICE();
+    FZ_FLUSH();
     const size_t B = (size_t)c->N * sizeof(double);
     const double *src[] = {u, v, w, p, phi, c->heat ? T : nullptr};
     double *dst[] = {c->u, c->v, c->w, c->p, c->phi, c->T};
@@ -540,6 +566,7 @@ extern "C" fizzy_status fizzy_get_fields(fizzy_ctx *c, double *u, double *v, dou
 {
     if (!c) return FIZZY_EINVAL;
     FZ_DEVICE();
+    FZ_FLUSH();
     const size_t B = (size_t)c->N * sizeof(double);
     double *dst[] = {u, v, w, p, phi, c->heat ? T : nullptr, p_prev};
     const double *src[] = {c->u, c->v, c->w, c->p, c->phi, c->T, c->pp};
@@ -567,10 +594,20 @@ extern "C" fizzy_status fizzy_rk3_substep(fizzy_ctx *c, int stage, double dt)
         k_latch_gamma<<<1, 1, 0, c->stream>>>(P, c->scal);
         FZ_LAUNCHED(FZK_LATCH);
     }
-    // S1: phi transport (divRn holds D(R/Gamma) of the current phi)
-    FZ_TB(FZK_PHI);
-    k_phi_update<<<grid, block, 0, c->stream>>>(P, c->phi, c->u, c->v, c->w, c->divrn, c->hphi, c->phin, c->psi, c->scal, dt, gs, zs, stage != 2);
-    FZ_LAUNCHED(FZK_PHI);
+    // S1: phi transport (divRn holds D(R/Gamma) of the current phi); with the S5 of the previous substep still
+    // pending it is fused in front (k_corr_phi)
+    if (c->corr_pending) {
+        FZ_TB(FZK_CORRPHI);
+        k_corr_phi<<<grid, block, 0, c->stream>>>(P, c->us, c->vs, c->ws, c->p, c->pp, c->phat, c->u, c->v, c->w, c->phi,
+                                                  c->divrn, c->hphi, c->phin, c->psi, c->scal, c->corr_coef, dt, gs, zs,
+                                                  stage != 2);
+        FZ_LAUNCHED(FZK_CORRPHI);
+        c->corr_pending = false;
+    } else {
+        FZ_TB(FZK_PHI);
+        k_phi_update<<<grid, block, 0, c->stream>>>(P, c->phi, c->u, c->v, c->w, c->divrn, c->hphi, c->phin, c->psi, c->scal, dt, gs, zs, stage != 2);
+        FZ_LAUNCHED(FZK_PHI);
+    }
     std::swap(c->phi, c->phin);
     // interface quantities of phi_new (N6): used by S3 now and by S1 of the next substep
     if ((s = run_interface(c, false)) != FIZZY_OK) return s;
@@ -598,14 +635,16 @@ extern "C" fizzy_status fizzy_rk3_substep(fizzy_ctx *c, int stage, double dt)
     if ((s = run_spectral_solve(c, c->pn)) != FIZZY_OK) return s;
     // S5: correction, pressure rotation
     // (rho1 != rho2: it also forms p_hat = 2 p_new - p for the next substep's predictor, N7)
-    FZ_TB(FZK_CORRECT);
-    if (stage == 2)
+    // after stages 0 and 1 it is deferred into the first kernel of the next substep (corr_pending)
+    if (stage == 2) {
+        FZ_TB(FZK_CORRECT);
         k_correct<true><<<grid, block, 0, c->stream>>>(P, c->us, c->vs, c->ws, c->pn, c->u, c->v, c->w,
                                                        as * dt / P.rho0, c->scal, c->p, c->phat);
-    else
-        k_correct<false><<<grid, block, 0, c->stream>>>(P, c->us, c->vs, c->ws, c->pn, c->u, c->v, c->w,
-                                                        as * dt / P.rho0, c->scal, c->p, c->phat);
-    FZ_LAUNCHED(FZK_CORRECT);
+        FZ_LAUNCHED(FZK_CORRECT);
+    } else {
+        c->corr_pending = true;
+        c->corr_coef = as * dt / P.rho0;
+    }
     double *old_pp = c->pp;
     c->pp = c->p;
     c->p = c->pn;
@@ -620,6 +659,7 @@ extern "C" fizzy_status fizzy_diagnostics(fizzy_ctx *c, double *out)
     FZ_DEVICE();
     if (!out) return fail(c, FIZZY_EINVAL, "out must be non-NULL");
     if (!c->fields_set) return fail(c, FIZZY_ESTATE, "fizzy_set_fields has not been called");
+    FZ_FLUSH();
     FZ_TB(FZK_OTHER);
     k_diag<<<FZ_DIAG_BLOCKS, 256, 0, c->stream>>>(c->P, c->u, c->v, c->w, c->phi, c->T, c->dpart);
     FZ_LAUNCHED(FZK_OTHER);
@@ -636,6 +676,7 @@ extern "C" fizzy_status fizzy_poisson_solve(fizzy_ctx *c, const double *rhs, dou
     if (!c) return FIZZY_EINVAL;
     FZ_DEVICE();
     if (!rhs || !p) return fail(c, FIZZY_EINVAL, "rhs and p must be non-NULL");
+    FZ_FLUSH();   // c->pn is the scratch of this call
     const FzP &P = c->P;
     const size_t B = (size_t)c->N * sizeof(double);
     FZ_CUDA(cudaMemcpyAsync(c->pn, rhs, B, cudaMemcpyDefault, c->stream));
@@ -654,6 +695,7 @@ extern "C" fizzy_status fizzy_check_finite(fizzy_ctx *c, long long *count)
     if (!c) return FIZZY_EINVAL;
     FZ_DEVICE();
     if (!count) return fail(c, FIZZY_EINVAL, "count must be non-NULL");
+    FZ_FLUSH();
     unsigned long long *cnt = reinterpret_cast<unsigned long long *>(c->scal + 5);
     FZ_CUDA(cudaMemsetAsync(cnt, 0, sizeof(*cnt), c->stream));
     FZ_TB(FZK_OTHER);
@@ -672,6 +714,7 @@ extern "C" fizzy_status fizzy_stable_dt(fizzy_ctx *c, double cfl, double *dt)
     FZ_DEVICE();
     if (!dt || !(cfl > 0.0)) return fail(c, FIZZY_EINVAL, "dt must be non-NULL and cfl > 0");
     if (!c->fields_set) return fail(c, FIZZY_ESTATE, "fizzy_set_fields has not been called");
+    FZ_FLUSH();
     const FzP &P = c->P;
     FZ_CUDA(cudaMemsetAsync(c->scal + 3, 0, 2 * sizeof(double), c->stream));
     FZ_TB(FZK_OTHER);

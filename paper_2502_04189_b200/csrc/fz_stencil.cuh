@@ -152,6 +152,62 @@ __global__ void k_phi_update(FzP P, const double *__restrict__ phi, const double
     psi[c] = P.eps * log(q);
 }
 
+// ---------------------------------------------------------------- S5 of the previous substep fused with S1
+// corrected face velocity  u = u** - (a dt / rho0) d_a p_new  (one spelling for k_correct and k_corr_phi: the value a
+// thread forms for a NEIGHBOUR's face is bit for bit the one the neighbour stores)
+__device__ __forceinline__ double fz_corr(double us, double coef, double p_hi, double p_lo, double ih)
+{
+    return us - coef * (p_hi - p_lo) * ih;
+}
+
+// After stages 0 and 1 the velocity correction is not launched on its own: the next substep starts with this kernel,
+// which forms u, v, w = u** - coef d(p_new) (stores them for S2b, S3) and uses them at once for the phi transport --
+// the corrected velocity is written but never read back by S1: -24 B/cell against k_correct + k_phi_update.
+// (After stage 2 k_correct runs on its own: Gamma of the next step needs max|u| before its S1, N15.)
+// phat != NULL (rho1 != rho2): also p_hat = 2 p_new - p_old (N7).
+__global__ void k_corr_phi(FzP P, const double *__restrict__ us, const double *__restrict__ vs,
+                           const double *__restrict__ ws, const double *__restrict__ pn,
+                           const double *__restrict__ pold, double *__restrict__ phat,
+                           double *__restrict__ u, double *__restrict__ v, double *__restrict__ w,
+                           const double *__restrict__ phi, const double *__restrict__ divrn,
+                           double *__restrict__ hphi, double *__restrict__ phin, double *__restrict__ psi,
+                           const double *__restrict__ scal, double coef, double dt, double gs, double zs, int keep_h)
+{
+    FZ_CELL_IJK
+    const FzZ z = fz_zn(P, k);
+    const unsigned nx = P.nx, sxy = (unsigned)P.sxy;
+    const unsigned pl = (unsigned)k * sxy, row = pl + nx * j, c = row + i;
+    const unsigned xp = row + fz_ip(i, P.nx), xm = row + fz_im(i, P.nx);
+    const unsigned yp = pl + nx * fz_ip(j, P.ny) + i, ym = pl + nx * fz_im(j, P.ny) + i;
+    const unsigned zp = (unsigned)z.kp * sxy + nx * j + i, zm = (unsigned)z.km * sxy + nx * j + i;
+    const double p0 = pn[c];
+    if (phat) phat[c] = 2.0 * p0 - pold[c];
+    // S5 at the cell's own three faces ...
+    const double un = fz_corr(us[c], coef, pn[xp], p0, P.idx);
+    const double vn = fz_corr(vs[c], coef, pn[yp], p0, P.idy);
+    const double wn = k < P.kzf ? fz_corr(ws[c], coef, pn[zp], p0, P.idzc[k]) : 0.0;
+    u[c] = un;
+    v[c] = vn;
+    w[c] = wn;
+    // ... and at the three faces below it (stored by the neighbours)
+    const double uxm = fz_corr(us[xm], coef, p0, pn[xm], P.idx);
+    const double vym = fz_corr(vs[ym], coef, p0, pn[ym], P.idy);
+    const double wzm = z.gm ? 0.0 : fz_corr(ws[zm], coef, p0, pn[zm], P.idzc[z.km]);
+    // S1 (as k_phi_update)
+    const double f0 = phi[c];
+    const double Fxp = -un * 0.5 * (f0 + phi[xp]), Fxm = -uxm * 0.5 * (phi[xm] + f0);
+    const double Fyp = -vn * 0.5 * (f0 + phi[yp]), Fym = -vym * 0.5 * (phi[ym] + f0);
+    const double Fzp = z.gp ? 0.0 : -wn * 0.5 * (f0 + phi[zp]);
+    const double Fzm = z.gm ? 0.0 : -wzm * 0.5 * (phi[zm] + f0);
+    const double rhs = (Fxp - Fxm) * P.idx + (Fyp - Fym) * P.idy + (Fzp - Fzm) * P.idzf[k] + scal[1] * divrn[c];
+    const double fn = f0 + dt * (gs * rhs + (zs != 0.0 ? zs * hphi[c] : 0.0));
+    phin[c] = fn;
+    if (keep_h) hphi[c] = rhs;
+    const double ph = fz_clip01(fn);
+    const double q = (ph + P.delta) / (1.0 - ph + P.delta);
+    psi[c] = P.eps * log(q);
+}
+
 // ---------------------------------------------------------------- S2b: temperature transport (N14)
 // RHS_T = D(-u_a Tbar_a) + D(kbar_a d_a T)/(rho cp), properties from phi_new;  k is linear in clip(phi),
 // so kbar_a = k2 + (k1-k2) * 0.5 (phic + phic(+1_a)).  32-bit offsets (N < 2^31), 8 CTAs/SM.
@@ -213,10 +269,10 @@ __global__ void k_correct(FzP P, const double *__restrict__ us, const double *__
     const long long c = i + P.nx * (j + pl);
     const double p0 = pn[c];
     if (phat) phat[c] = 2.0 * p0 - pold[c];
-    const double un = us[c] - coef * (pn[fz_ip(i, P.nx) + P.nx * (j + pl)] - p0) * P.idx;
-    const double vn = vs[c] - coef * (pn[i + P.nx * (fz_ip(j, P.ny) + pl)] - p0) * P.idy;
+    const double un = fz_corr(us[c], coef, pn[fz_ip(i, P.nx) + P.nx * (j + pl)], p0, P.idx);
+    const double vn = fz_corr(vs[c], coef, pn[i + P.nx * (fz_ip(j, P.ny) + pl)], p0, P.idy);
     double wn = 0.0;
-    if (k < P.kzf) wn = ws[c] - coef * (pn[c + (long long)(z.kp - k) * P.sxy] - p0) * P.idzc[k];
+    if (k < P.kzf) wn = fz_corr(ws[c], coef, pn[c + (long long)(z.kp - k) * P.sxy], p0, P.idzc[k]);
     u[c] = un;
     v[c] = vn;
     w[c] = wn;

@@ -66,6 +66,7 @@ struct fizzy_ctx {
     double *T, *Tn, *hT;
     double *kappa, *divrn, *psi, *rr, *nhx, *nhy, *nhz, *rnx, *rny, *rnz;
     double2 *spec;
+    CUtensorMap tm_spec;   // the half-spectrum as a rank-3 tensor (2 ny doubles | nxh | nz): input boxes of k_fftx_inv (TMA)
     double2 *twx, *twy;
     double *scal;  // [0] running max|u|, [1] Gamma, [2], [6] gauge mean (two parts), [3..4] dt maxima, [5] non-finite count, [8..15] diagnostics
     double dzmin;  // smallest cell height (N16)
@@ -314,12 +315,34 @@ extern "C" fizzy_status fizzy_create(const fizzy_grid *grid, const fizzy_bc *bc,
     k_tri_tables<<<(unsigned)((c->M + 127) / 128), 128, 0, c->stream>>>(P, c->tri);
     FZ_LAUNCHED(FZK_OTHER);
 
+    // ---- tensor map of the half-spectrum for the TMA loads of k_fftx_inv (driver entry point through the runtime:
+    // libfizzy.so does not link libcuda)
+    {
+        typedef CUresult (*encode_fn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                      const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
+                                      CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+        void *fn = nullptr;
+        cudaDriverEntryPointQueryResult qres;
+        FZ_CUDA(cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres));
+        if (!fn || qres != cudaDriverEntryPointSuccess) return fail(c, FIZZY_ECUDA, "cuTensorMapEncodeTiled is not available");
+        const FzFxInvGeom G = fx_inv_geom(c->log2nx);
+        const cuuint64_t gdim[3] = {(cuuint64_t)2 * ny, (cuuint64_t)P.nxh, (cuuint64_t)nz};
+        const cuuint64_t gstr[2] = {(cuuint64_t)ny * 16, (cuuint64_t)P.nxh * ny * 16};
+        const cuuint32_t box[3] = {(cuuint32_t)(G.rowb / 8), (cuuint32_t)G.brows, 1};
+        const cuuint32_t estr[3] = {1, 1, 1};
+        const CUtensorMapSwizzle sw = G.rowb == 128 ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_64B;
+        const CUresult r = reinterpret_cast<encode_fn>(fn)(&c->tm_spec, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, c->spec, gdim, gstr,
+                                                           box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, sw,
+                                                           CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+        if (r != CUDA_SUCCESS) return fail(c, FIZZY_ECUDA, "cuTensorMapEncodeTiled failed");
+    }
+
     // dynamic shared memory opt-in of every kernel instantiation this context will launch: once, here,
     // so that a substep is launches only (and can be captured into a CUDA graph)
     FZ_CUDA(cudaFuncSetAttribute(k_iface_march<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)IFACE_SMEM));
     FZ_CUDA(cudaFuncSetAttribute(k_iface_march<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)IFACE_SMEM));
     FZ_CUDA(launch_momentum(c, dim3(), dim3(), nullptr));
-    FZ_CUDA(fz_fftx_launch(-1, c->log2nx, P, nullptr, nullptr, nullptr, nullptr, 0.0, nullptr, nullptr, nullptr, nullptr, c->stream));
+    FZ_CUDA(fz_fftx_launch(-1, c->log2nx, P, nullptr, nullptr, nullptr, nullptr, 0.0, nullptr, nullptr, nullptr, nullptr, nullptr, c->stream));
     FZ_CUDA(c->cyclic ? fz_spec_launch<true>(-1, c->log2ny, P, c->tri, nullptr, nullptr, nullptr, c->stream)
                       : fz_spec_launch<false>(-1, c->log2ny, P, c->tri, nullptr, nullptr, nullptr, c->stream));
     return FIZZY_OK;
@@ -443,7 +466,7 @@ fizzy_status run_spectral_solve(fizzy_ctx *c, double *dst)
     FZ_LAUNCHED(FZK_SPEC_BWD);
     FZ_TB(FZK_FFTX_INV);
     FZ_CUDA(fz_fftx_launch(2, c->log2nx, P, nullptr, nullptr, nullptr, nullptr, 1.0 / ((double)P.nx * (double)P.ny),
-                           c->spec, dst, c->twx, c->scal, c->stream));
+                           c->spec, dst, c->twx, c->scal, &c->tm_spec, c->stream));
     FZ_LAUNCHED(FZK_FFTX_INV);
     return FIZZY_OK;
 }
@@ -630,7 +653,7 @@ extern "C" fizzy_status fizzy_rk3_substep(fizzy_ctx *c, int stage, double dt)
     // S4: b = rho0/(a dt) D(u**), FFT x (fused), FFT y, tridiagonal z, inverse
     FZ_TB(FZK_FFTX_FWD);
     FZ_CUDA(fz_fftx_launch(0, c->log2nx, P, nullptr, c->us, c->vs, c->ws, P.rho0 / (as * dt), c->spec, nullptr,
-                           c->twx, c->scal, c->stream));
+                           c->twx, c->scal, nullptr, c->stream));
     FZ_LAUNCHED(FZK_FFTX_FWD);
     if ((s = run_spectral_solve(c, c->pn)) != FIZZY_OK) return s;
     // S5: correction, pressure rotation
@@ -682,7 +705,7 @@ extern "C" fizzy_status fizzy_poisson_solve(fizzy_ctx *c, const double *rhs, dou
     FZ_CUDA(cudaMemcpyAsync(c->pn, rhs, B, cudaMemcpyDefault, c->stream));
     FZ_TB(FZK_FFTX_FWD);
     FZ_CUDA(fz_fftx_launch(1, c->log2nx, P, c->pn, nullptr, nullptr, nullptr, 1.0, c->spec, nullptr, c->twx, c->scal,
-                           c->stream));
+                           nullptr, c->stream));
     FZ_LAUNCHED(FZK_FFTX_FWD);
     fizzy_status s = run_spectral_solve(c, c->pn);
     if (s != FIZZY_OK) return s;

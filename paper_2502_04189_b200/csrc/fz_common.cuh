@@ -100,3 +100,32 @@ __device__ __forceinline__ void fz_cp_async8(void *smem_dst, const void *gsrc)
 __device__ __forceinline__ void fz_cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 template <int N>
 __device__ __forceinline__ void fz_cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+
+// ---------------------------------------------------------------- TMA (cp.async.bulk.tensor) and mbarrier
+// One elected thread initialises the barrier, announces the byte count and issues the tensor copies; every thread
+// then waits for the phase to flip.  The tensor map is built on the host (fizzy_create, cuTensorMapEncodeTiled).
+__device__ __forceinline__ unsigned fz_smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void fz_mbar_init(void *bar, unsigned count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(fz_smem_u32(bar)), "r"(count) : "memory");
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+}
+__device__ __forceinline__ void fz_mbar_expect_tx(void *bar, unsigned bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(fz_smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void fz_mbar_wait(void *bar, unsigned phase)
+{
+    unsigned done;
+    do {
+        asm volatile("{\n\t.reg .pred P1;\n\tmbarrier.try_wait.parity.shared::cta.b64 P1, [%1], %2;\n\tselp.b32 %0, 1, 0, P1;\n\t}"
+                     : "=r"(done) : "r"(fz_smem_u32(bar)), "r"(phase) : "memory");
+    } while (!done);
+}
+// box of a rank-3 tensor map -> shared memory; coordinates innermost first
+__device__ __forceinline__ void fz_tma_load_3d(void *smem_dst, const void *tmap, int c0, int c1, int c2, void *bar)
+{
+    asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];"
+                 ::"r"(fz_smem_u32(smem_dst)), "l"(tmap), "r"(fz_smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2) : "memory");
+}

@@ -11,6 +11,7 @@
 //   b = coef * D(u**)  (BASELINE.json:5(iv) with the p_hat term folded into u**, D2);
 // DIV = false: the real input is read from `src` (fizzy_poisson_solve).
 #pragma once
+#include <cuda.h>
 #include "fz_common.cuh"
 #include "fz_linefft.cuh"
 
@@ -89,47 +90,74 @@ k_fftx_fwd(FzP P, const double *__restrict__ src, const double *__restrict__ us,
 
 // ---------------------------------------------------------------- FFT along x, backward (c2r)
 // out = Re / Im of the inverse transform * scale - gauge shift (N17: scal[2] + scal[6] = mean of mode (0,0),
-// written by k_spec_bwd)
+// written by k_spec_bwd).
+// The CTA's input is, for every x-mode l, a run of 2*FX_PAIRS consecutive j of the spectrum: nxh pieces of 128 (64)
+// bytes, 16*ny bytes apart.  Read by the threads themselves these scattered pieces kept the LSU data pipe 87 % busy
+// with DRAM at 53 % (ncu r2a).  They are one BOX of a rank-3 tensor (2 ny doubles | nxh | nz), so ONE thread fetches
+// them with TMA (cp.async.bulk.tensor, boxes of at most 256 rows, 128-byte swizzle, completion on an mbarrier) into
+// a staging area [l][2*FX_PAIRS]; every thread then takes the eight inputs of its first radix-8 pass straight from
+// there, tangling on the fly (rows l <= n/2 directly, the others from the mirror row n-l) -- no tangle pass through
+// shared memory, no barrier before the transform.  The staging area aliases the second FFT buffer, which the transform
+// writes only after the barrier that follows its first pass.
+struct FzFxInvGeom {   // staging geometry, the same on the host (tensor map) and in the kernel
+    int pairs, rowb, nbox, brows, swz;   // bytes per staged row, boxes, rows per box, swizzle mask (16-byte chunks)
+};
+__host__ __device__ constexpr FzFxInvGeom fx_inv_geom(int log2n)
+{
+    const int pairs = fx_pairs(log2n, true), nxh = (1 << log2n) / 2 + 1;
+    const int rowb = pairs * 32, nbox = (nxh + 255) / 256;
+    const int brows = ((nxh + nbox - 1) / nbox + 7) / 8 * 8;   // a multiple of 8 rows: every box starts on a swizzle period
+    return FzFxInvGeom{pairs, rowb, nbox, brows, rowb / 16 - 1};
+}
+__host__ __device__ constexpr size_t fx_inv_smem(int log2n)
+{
+    const FzFxInvGeom G = fx_inv_geom(log2n);
+    const size_t buf = (size_t)G.pairs * FX_LINE(1 << log2n) * 16, stage = (size_t)G.nbox * G.brows * G.rowb;
+    return ((buf > stage ? buf : stage) + 127) / 128 * 128 + buf;   // [Y | staging][X]
+}
+
 template <int LOG2N>
 __global__ void __launch_bounds__(fx_pairs(LOG2N, true) * ((1 << LOG2N) / 8), fx_minb(LOG2N, true))
-k_fftx_inv(FzP P, const double2 *__restrict__ spec, double *__restrict__ dst, double scale,
+k_fftx_inv(FzP P, const __grid_constant__ CUtensorMap tm_spec, double *__restrict__ dst, double scale,
            const double2 *__restrict__ tw, const double *__restrict__ scal)
 {
-    extern __shared__ __align__(16) double2 smx[];
-    constexpr int n = 1 << LOG2N, T8 = n / 8, LN = FX_LINE(n), PS = FX_PAIR(n), FX_PAIRS = fx_pairs(LOG2N, true);
-    const int jt = threadIdx.x, g = threadIdx.y;
-    double2 *A = smx + g * PS, *B = A + LN;
+    extern __shared__ __align__(1024) unsigned char smb[];
+    __shared__ __align__(8) unsigned long long bar;
+    constexpr int n = 1 << LOG2N, T8 = n / 8, LN = FX_LINE(n);
+    constexpr FzFxInvGeom G = fx_inv_geom(LOG2N);
+    constexpr size_t YB = fx_inv_smem(LOG2N) - (size_t)G.pairs * LN * 16;
+    const int jt = threadIdx.x, g = threadIdx.y, t = g * T8 + jt;
+    double2 *Y = reinterpret_cast<double2 *>(smb) + g * LN, *X = reinterpret_cast<double2 *>(smb + YB) + g * LN;
+    const long long L0 = (long long)blockIdx.x * (2 * G.pairs);
+    const int k = (int)(L0 / P.ny), j0 = (int)(L0 - (long long)k * P.ny);
+    if (t == 0) fz_mbar_init(&bar, 1);
+    __syncthreads();
+    if (t == 0) {
+        fz_mbar_expect_tx(&bar, (unsigned)(G.nbox * G.brows * G.rowb));
+#pragma unroll
+        for (int b = 0; b < G.nbox; ++b)   // rows past nxh are outside the tensor: filled with zeros, never read
+            fz_tma_load_3d(smb + (size_t)b * G.brows * G.rowb, &tm_spec, 2 * j0, b * G.brows, k, &bar);
+    }
     FzLineFFT<LOG2N, +1, false> fft;
     fft.init(tw, jt);
-    const long long L0 = (long long)blockIdx.x * (2 * FX_PAIRS);
-    const int k = (int)(L0 / P.ny), j0 = (int)(L0 - (long long)k * P.ny);
     const double shift = (scal[2] + scal[6]) * scale;
-    const int nth = T8 * FX_PAIRS, t = g * T8 + jt;
-    const int nxh = P.nxh;
-    const double2 *in = spec + (long long)k * nxh * P.ny + j0;
-    {   // L2 prefetch of the spectrum rows of the CTA FX_AHEAD launches later (2*FX_PAIRS*16 bytes per l)
-        const long long Lp = L0 + (long long)FX_AHEAD * (2 * FX_PAIRS);
-        if (Lp < (long long)P.ny * P.nz) {
-            const int kp = (int)(Lp / P.ny), jp = (int)(Lp - (long long)kp * P.ny);
-            const double2 *inp = spec + (long long)kp * nxh * P.ny + jp;
-            for (int l = t; l < nxh; l += nth) fz_prefetch_l2(inp + (long long)l * P.ny);
-        }
-    }
-    // tangle: consecutive threads -> consecutive pairs (32-byte pieces, runs of 2*FX_PAIRS*16 bytes per l)
-    for (int e = t; e < FX_PAIRS * nxh; e += nth) {
-        const int l = e / FX_PAIRS, pr = e - l * FX_PAIRS;
-        const double2 a = in[(long long)l * P.ny + 2 * pr], b = in[(long long)l * P.ny + 2 * pr + 1];
-        double2 *buf = smx + pr * PS;
-        if (l == 0 || l == n / 2) {
-            buf[FZL_PADI(l)] = make_double2(a.x, b.x);
-        } else {
-            buf[FZL_PADI(l)] = make_double2(a.x - b.y, a.y + b.x);
-            buf[FZL_PADI(n - l)] = make_double2(a.x + b.y, b.x - a.y);
-        }
-    }
-    __syncthreads();
+    fz_mbar_wait(&bar, 0);
+    // inputs of the first pass: Z_l = A_l + i B_l (l <= n/2), Z_l = conj(A_{n-l}) + i conj(B_{n-l}) (l > n/2); the
+    // pair's A_l, B_l are the 16-byte chunks 2g, 2g+1 of staged row l (chunk index XOR row: the TMA swizzle)
     double2 v[8];
-    fft.smem_to_regs(jt, A, B, v);
+#pragma unroll
+    for (int r = 0; r < 8; ++r) {
+        const int l = jt + r * T8;
+        const bool mir = l > n / 2;
+        const int row = mir ? n - l : l;
+        unsigned off = (unsigned)row * G.rowb + 32u * g;
+        off ^= ((off >> 7) & G.swz) << 4;
+        const double2 a = *reinterpret_cast<const double2 *>(smb + off), b = *reinterpret_cast<const double2 *>(smb + (off ^ 16u));
+        if (mir) v[r] = make_double2(a.x + b.y, b.x - a.y);
+        else if (l == 0 || l == n / 2) v[r] = make_double2(a.x, b.x);
+        else v[r] = make_double2(a.x - b.y, a.y + b.x);
+    }
+    fft.regs_to_regs(jt, X, Y, v);
     const int ja = j0 + 2 * g;
     const long long ra = ((long long)k * P.ny + ja) * n, rb = ra + n;
 #pragma unroll
@@ -145,10 +173,11 @@ k_fftx_inv(FzP P, const double2 *__restrict__ spec, double *__restrict__ dst, do
 template <int LOG2N>
 cudaError_t fz_fftx_launch_one(int which /*0 fwd DIV, 1 fwd plain, 2 inv*/, const FzP &P, const double *src,
                                const double *us, const double *vs, const double *ws, double coef, double2 *spec,
-                               double *dst, const double2 *tw, const double *scal, cudaStream_t st)
+                               double *dst, const double2 *tw, const double *scal, const CUtensorMap *tm_spec,
+                               cudaStream_t st)
 {
     if (which < 0) {
-        const int sf = (int)fz_fftx_smem(LOG2N, false), si = (int)fz_fftx_smem(LOG2N, true);
+        const int sf = (int)fz_fftx_smem(LOG2N, false), si = (int)fx_inv_smem(LOG2N);
         cudaError_t e = cudaFuncSetAttribute(k_fftx_fwd<true, LOG2N>, cudaFuncAttributeMaxDynamicSharedMemorySize, sf);
         if (e == cudaSuccess) e = cudaFuncSetAttribute(k_fftx_fwd<false, LOG2N>, cudaFuncAttributeMaxDynamicSharedMemorySize, sf);
         if (e == cudaSuccess) e = cudaFuncSetAttribute(k_fftx_inv<LOG2N>, cudaFuncAttributeMaxDynamicSharedMemorySize, si);
@@ -156,21 +185,21 @@ cudaError_t fz_fftx_launch_one(int which /*0 fwd DIV, 1 fwd plain, 2 inv*/, cons
     }
     const int n = 1 << LOG2N;
     const int np = fx_pairs(LOG2N, which == 2);
-    const size_t smem = fz_fftx_smem(LOG2N, which == 2);
+    const size_t smem = which == 2 ? fx_inv_smem(LOG2N) : fz_fftx_smem(LOG2N, false);
     const dim3 block(n / 8, np);
     const unsigned grid = (unsigned)(((long long)P.ny * P.nz) / (2 * np));
     if (which == 0) k_fftx_fwd<true, LOG2N><<<grid, block, smem, st>>>(P, nullptr, us, vs, ws, coef, spec, tw);
     else if (which == 1) k_fftx_fwd<false, LOG2N><<<grid, block, smem, st>>>(P, src, nullptr, nullptr, nullptr, 1.0, spec, tw);
-    else k_fftx_inv<LOG2N><<<grid, block, smem, st>>>(P, spec, dst, coef, tw, scal);
+    else k_fftx_inv<LOG2N><<<grid, block, smem, st>>>(P, *tm_spec, dst, coef, tw, scal);
     return cudaSuccess;
 }
 
 inline cudaError_t fz_fftx_launch(int which, int log2n, const FzP &P, const double *src, const double *us,
                                   const double *vs, const double *ws, double coef, double2 *spec, double *dst,
-                                  const double2 *tw, const double *scal, cudaStream_t st)
+                                  const double2 *tw, const double *scal, const CUtensorMap *tm_spec, cudaStream_t st)
 {
     switch (log2n) {
-#define FZ_CASE(L_) case L_: return fz_fftx_launch_one<L_>(which, P, src, us, vs, ws, coef, spec, dst, tw, scal, st);
+#define FZ_CASE(L_) case L_: return fz_fftx_launch_one<L_>(which, P, src, us, vs, ws, coef, spec, dst, tw, scal, tm_spec, st);
         FZ_CASE(3) FZ_CASE(4) FZ_CASE(5) FZ_CASE(6) FZ_CASE(7) FZ_CASE(8) FZ_CASE(9) FZ_CASE(10)
 #undef FZ_CASE
     }

@@ -159,4 +159,24 @@ struct FzLineFFT {
         }
         return cur;
     }
+    // Input element jt + r*T8 in v[r] (registers), output element jt + q*T8 in v[q].  Pass 0 writes X; Y is written
+    // only after the barrier that follows pass 0, so the caller's inputs may live in memory that Y aliases.
+    __device__ __forceinline__ void regs_to_regs(int jt, double2 *X, double2 *Y, double2 (&v)[8]) const
+    {
+        if (OUT_IN_REGS && NP8 == 1) { pass8<true, true>(0, jt, v, Y, X); return; }
+        pass8<true, false>(0, jt, v, Y, X);
+        sync();
+        double2 *cur = X, *oth = Y;
+#pragma unroll
+        for (int p = 1; p < NP8; ++p) {
+            if (OUT_IN_REGS && p == NP8 - 1) { pass8<false, true>(p, jt, v, cur, oth); return; }
+            pass8<false, false>(p, jt, v, cur, oth);
+            sync();
+            double2 *t = cur; cur = oth; oth = t;
+        }
+        passr(jt, cur, oth);
+        sync();
+#pragma unroll
+        for (int q = 0; q < 8; ++q) v[q] = oth[FZL_PADI(jt + q * T8)];
+    }
 };

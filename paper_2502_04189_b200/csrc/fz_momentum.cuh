@@ -357,24 +357,27 @@ k_momentum_march(FzP P, FzMomArgs A, int KC)
         // edge viscosity (N11): mean of the four cells around the edge; a constant if mu1 == mu2
 #define MUE_(a_, b_, c_, d_) (VARMU ? 0.25 * ((a_) + (b_) + (c_) + (d_)) : P.mu2)
         // advective edge products and edge stresses on the three "+" edges of the cell, shared by
-        // the two components that meet there
-        const double Exy_p = 0.5 * (v000 + vp00) * 0.5 * (u000 + u0p0);
-        const double Exz_p = 0.5 * (w000 + wp00) * 0.5 * (u000 + u00p);
-        const double Eyz_p = 0.5 * (w000 + w0p0) * 0.5 * (v000 + v00p);
+        // the two components that meet there.  The halves of the face averages are folded into the metric factors
+        // (q* = 1/4 of the reciprocal spacing): E' = (sum of two)(sum of two), uc' = sum of two.
+        const double qx = 0.25 * dx, qy = 0.25 * dy, qzf = 0.25 * izf, qzc = 0.25 * izc;
+        const double Exy_p = (v000 + vp00) * (u000 + u0p0);
+        const double Exz_p = (w000 + wp00) * (u000 + u00p);
+        const double Eyz_p = (w000 + w0p0) * (v000 + v00p);
         const double txy_p = MUE_(m000, mp00, m0p0, mpp0) * ((u0p0 - u000) * dy + (vp00 - v000) * dx);
         const double txz_p = MUE_(m000, mp00, m00p, mp0p) * ((u00p - u000) * izc + (wp00 - w000) * dx);
         const double tyz_p = MUE_(m000, m0p0, m00p, m0pp) * ((v00p - v000) * izc + (w0p0 - w000) * dy);
+        const double hs = 0.5 * P.sigma;
         // ================= x component =================
         {
-            const double uc_p = 0.5 * (up00 + u000), uc_m = 0.5 * (u000 + um00);
-            const double Exy_m = 0.5 * (v0m0 + vpm0) * 0.5 * (u0m0 + u000);
-            const double Exz_m = 0.5 * (w00m + wp0m) * 0.5 * (u00m + u000);
-            const double Aa = -(uc_p * uc_p - uc_m * uc_m) * dx - (Exy_p - Exy_m) * dy - (Exz_p - Exz_m) * izf;
-            const double nrm_p = 2.0 * mp00 * (up00 - u000) * dx, nrm_m = 2.0 * m000 * (u000 - um00) * dx;
+            const double uc_p = up00 + u000, uc_m = u000 + um00;
+            const double Exy_m = (v0m0 + vpm0) * (u0m0 + u000);
+            const double Exz_m = (w00m + wp0m) * (u00m + u000);
+            const double Aa = -((uc_p * uc_p - uc_m * uc_m) * qx + (Exy_p - Exy_m) * qy + (Exz_p - Exz_m) * qzf);
+            const double nrm_p = mp00 * (up00 - u000), nrm_m = m000 * (u000 - um00);
             const double txy_m = MUE_(m0m0, mpm0, m000, mp00) * ((u000 - u0m0) * dy + (vpm0 - v0m0) * dx);
             const double txz_m = MUE_(m00m, mp0m, m000, mp00) * ((u000 - u00m) * izcm + (wp0m - w00m) * dx);
-            const double V = (nrm_p - nrm_m) * dx + (txy_p - txy_m) * dy + (txz_p - txz_m) * izf;
-            const double Sf = P.sigma * 0.5 * (kap0 + S_(F::KAP, 1, 0, o0)) * (fp00 - f000) * dx;
+            const double V = (nrm_p - nrm_m) * (2.0 * dx * dx) + (txy_p - txy_m) * dy + (txz_p - txz_m) * izf;
+            const double Sf = (hs * dx) * (kap0 + S_(F::KAP, 1, 0, o0)) * (fp00 - f000);
             double M = 0.0;
             if (VARRHO) {
                 const double Rty = 0.25 * (S_(F::RY, 0, 0, o0) + S_(F::RY, 1, 0, o0) + S_(F::RY, 0, -1, o0) + S_(F::RY, 1, -1, o0));
@@ -392,17 +395,17 @@ k_momentum_march(FzP P, FzMomArgs A, int KC)
         }
         // ================= y component =================
         {
-            const double vc_p = 0.5 * (v0p0 + v000), vc_m = 0.5 * (v000 + v0m0);
+            const double vc_p = v0p0 + v000, vc_m = v000 + v0m0;
             const double Eyx_p = Exy_p;
-            const double Eyx_m = 0.5 * (um00 + ump0) * 0.5 * (vm00 + v000);
-            const double Eyz_m = 0.5 * (w00m + w0pm) * 0.5 * (v00m + v000);
-            const double Aa = -(vc_p * vc_p - vc_m * vc_m) * dy - (Eyx_p - Eyx_m) * dx - (Eyz_p - Eyz_m) * izf;
-            const double nrm_p = 2.0 * m0p0 * (v0p0 - v000) * dy, nrm_m = 2.0 * m000 * (v000 - v0m0) * dy;
+            const double Eyx_m = (um00 + ump0) * (vm00 + v000);
+            const double Eyz_m = (w00m + w0pm) * (v00m + v000);
+            const double Aa = -((vc_p * vc_p - vc_m * vc_m) * qy + (Eyx_p - Eyx_m) * qx + (Eyz_p - Eyz_m) * qzf);
+            const double nrm_p = m0p0 * (v0p0 - v000), nrm_m = m000 * (v000 - v0m0);
             const double tyx_p = txy_p;
             const double tyx_m = MUE_(mm00, mmp0, m000, m0p0) * ((v000 - vm00) * dx + (ump0 - um00) * dy);
             const double tyz_m = MUE_(m00m, m0pm, m000, m0p0) * ((v000 - v00m) * izcm + (w0pm - w00m) * dy);
-            const double V = (nrm_p - nrm_m) * dy + (tyx_p - tyx_m) * dx + (tyz_p - tyz_m) * izf;
-            const double Sf = P.sigma * 0.5 * (kap0 + S_(F::KAP, 0, 1, o0)) * (f0p0 - f000) * dy;
+            const double V = (nrm_p - nrm_m) * (2.0 * dy * dy) + (tyx_p - tyx_m) * dx + (tyz_p - tyz_m) * izf;
+            const double Sf = (hs * dy) * (kap0 + S_(F::KAP, 0, 1, o0)) * (f0p0 - f000);
             double M = 0.0;
             if (VARRHO) {
                 const double Rtx = 0.25 * (S_(F::RX, 0, 0, o0) + S_(F::RX, 0, 1, o0) + S_(F::RX, -1, 0, o0) + S_(F::RX, -1, 1, o0));
@@ -421,19 +424,19 @@ k_momentum_march(FzP P, FzMomArgs A, int KC)
         // ================= z component =================
         if (k < P.kzf) {
             const double w00p = S_(F::W, 0, 0, op);
-            const double wc_p = 0.5 * (w00p + w000), wc_m = 0.5 * (w000 + w00m);
+            const double wc_p = w00p + w000, wc_m = w000 + w00m;
             const double Ezx_p = Exz_p;
-            const double Ezx_m = 0.5 * (um00 + um0p) * 0.5 * (wm00 + w000);
+            const double Ezx_m = (um00 + um0p) * (wm00 + w000);
             const double Ezy_p = Eyz_p;
-            const double Ezy_m = 0.5 * (v0m0 + v0mp) * 0.5 * (w0m0 + w000);
-            const double Aa = -(wc_p * wc_p - wc_m * wc_m) * izc - (Ezx_p - Ezx_m) * dx - (Ezy_p - Ezy_m) * dy;
-            const double nrm_p = 2.0 * m00p * (w00p - w000) * izfp, nrm_m = 2.0 * m000 * (w000 - w00m) * izf;
+            const double Ezy_m = (v0m0 + v0mp) * (w0m0 + w000);
+            const double Aa = -((wc_p * wc_p - wc_m * wc_m) * qzc + (Ezx_p - Ezx_m) * qx + (Ezy_p - Ezy_m) * qy);
+            const double nrm_p = m00p * (w00p - w000) * izfp, nrm_m = m000 * (w000 - w00m) * izf;
             const double tzx_p = txz_p;
             const double tzx_m = MUE_(mm00, mm0p, m000, m00p) * ((w000 - wm00) * dx + (um0p - um00) * izc);
             const double tzy_p = tyz_p;
             const double tzy_m = MUE_(m0m0, m0mp, m000, m00p) * ((w000 - w0m0) * dy + (v0mp - v0m0) * izc);
-            const double V = (nrm_p - nrm_m) * izc + (tzx_p - tzx_m) * dx + (tzy_p - tzy_m) * dy;
-            const double Sf = P.sigma * 0.5 * (kap0 + S_(F::KAP, 0, 0, op)) * (f00p - f000) * izc;
+            const double V = (nrm_p - nrm_m) * (2.0 * izc) + (tzx_p - tzx_m) * dx + (tzy_p - tzy_m) * dy;
+            const double Sf = (hs * izc) * (kap0 + S_(F::KAP, 0, 0, op)) * (f00p - f000);
             double M = 0.0;
             if (VARRHO) {
                 const double Rtx = 0.25 * (S_(F::RX, 0, 0, o0) + S_(F::RX, 0, 0, op) + S_(F::RX, -1, 0, o0) + S_(F::RX, -1, 0, op));

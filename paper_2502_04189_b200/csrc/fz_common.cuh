@@ -25,6 +25,11 @@ struct FzP {
 };
 
 __device__ __forceinline__ double fz_clip01(double f) { return fmin(fmax(f, 0.0), 1.0); }
+// 2 clip(f,0,1) - 1 = |f| - |f - 1| without a comparison (two DADD with operand modifiers instead of DSETP + selects
+// + moves per fmin/fmax): exact outside [0,1], within one rounding of 1 (1.1e-16 ABSOLUTE) inside.  For the linear
+// property maps q2 + (q1-q2) clip(phi) = (q2+q1)/2 + (q1-q2)/2 * fz_sclip(phi), where an absolute error of that size
+// is the rounding error of the map itself; NOT for psi, which needs tiny phi to full relative accuracy.
+__device__ __forceinline__ double fz_sclip(double f) { return fabs(f) - fabs(f - 1.0); }
 
 // neighbour indices of a cell in the periodic directions
 __device__ __forceinline__ int fz_ip(int i, int n) { return (i + 1 == n) ? 0 : i + 1; }

@@ -270,7 +270,8 @@ k_momentum_march(FzP P, FzMomArgs A, int KC)
     for (int d = 1; d <= MRING - 3; ++d) { issue(k0 + d); fz_cp_async_commit(); }
 
     const double dx = P.idx, dy = P.idy;
-    const double dmu = P.mu1 - P.mu2;
+    const double hdmu = 0.5 * (P.mu1 - P.mu2), mumid = 0.5 * (P.mu1 + P.mu2);
+    const double qdrho = 0.25 * P.drho, rhomid = 0.5 * (P.rho1 + P.rho2);
     const double ir0 = 1.0 / P.rho0;
     const double Gam = A.scal[1];
 
@@ -319,7 +320,7 @@ k_momentum_march(FzP P, FzMomArgs A, int KC)
                      f00p = S_(F::PHI, 0, 0, op);
         double m000, mp00, mm00, m0p0, m0m0, m00p, m00m, mpp0, mpm0, mmp0, mp0p, mp0m, mm0p, m0pp, m0pm, m0mp;
         if (VARMU) {
-#define FZ_MU(x) (P.mu2 + dmu * fz_clip01(x))
+#define FZ_MU(x) fma(hdmu, fz_sclip(x), mumid)
             m000 = FZ_MU(f000); mp00 = FZ_MU(fp00); m0p0 = FZ_MU(f0p0); m00p = FZ_MU(f00p);
             mm00 = FZ_MU(S_(F::PHI, -1, 0, o0)); m0m0 = FZ_MU(S_(F::PHI, 0, -1, o0)); m00m = FZ_MU(S_(F::PHI, 0, 0, om));
             mpp0 = FZ_MU(S_(F::PHI, 1, 1, o0)); mpm0 = FZ_MU(S_(F::PHI, 1, -1, o0)); mmp0 = FZ_MU(S_(F::PHI, -1, 1, o0));
@@ -334,10 +335,11 @@ k_momentum_march(FzP P, FzMomArgs A, int KC)
         double irx = 1.0 / P.rho2, iry = irx, irz = irx;
         double ph000 = 0, php00 = 0, ph0p0 = 0, ph00p = 0;
         if (VARRHO) {
-            const double r000 = P.rho2 + P.drho * fz_clip01(f000);
-            irx = fz_rcp(0.5 * (r000 + P.rho2 + P.drho * fz_clip01(fp00)));
-            iry = fz_rcp(0.5 * (r000 + P.rho2 + P.drho * fz_clip01(f0p0)));
-            irz = fz_rcp(0.5 * (r000 + P.rho2 + P.drho * fz_clip01(f00p)));
+            // rho_f = 1/2 (rho + rho(+1_a)) = rhomid + 1/4 drho (sclip + sclip(+1_a))   (fz_sclip: 2 clip - 1)
+            const double s000 = fz_sclip(f000);
+            irx = fz_rcp(fma(qdrho, s000 + fz_sclip(fp00), rhomid));
+            iry = fz_rcp(fma(qdrho, s000 + fz_sclip(f0p0), rhomid));
+            irz = fz_rcp(fma(qdrho, s000 + fz_sclip(f00p), rhomid));
             // p_hat = 2 p - p_prev (N7), formed by k_correct of the previous substep
             ph000 = S_(F::PH, 0, 0, o0); php00 = S_(F::PH, 1, 0, o0); ph0p0 = S_(F::PH, 0, 1, o0);
             ph00p = S_(F::PH, 0, 0, op);

@@ -224,29 +224,31 @@ k_temp_update(FzP P, const double *__restrict__ T, const double *__restrict__ ph
     const unsigned xp = row + fz_ip(i, P.nx), xm = row + fz_im(i, P.nx);
     const unsigned yp = pl + nx * fz_ip(j, P.ny) + i, ym = pl + nx * fz_im(j, P.ny) + i;
     const unsigned zp = (unsigned)z.kp * sxy + nx * j + i, zm = (unsigned)z.km * sxy + nx * j + i;
-    const double hdk = 0.5 * (P.k1 - P.k2);
-    const double t0 = T[c], phc = fz_clip01(phi[c]);
+    // face conductivity kbar_a = kmid + 1/4 (k1-k2) (sclip + sclip(+1_a)), fz_sclip = 2 clip - 1 (no comparisons)
+    const double qdk = 0.25 * (P.k1 - P.k2), kmid = 0.5 * (P.k1 + P.k2);
+    const double t0 = T[c], s0 = fz_sclip(phi[c]);
     const double izf = P.idzf[k], idx = P.idx, idy = P.idy;
     double adv, dif;
     {   // x
         const double tp = T[xp], tm = T[xm];
-        const double kp = P.k2 + hdk * (phc + fz_clip01(phi[xp])), km = P.k2 + hdk * (fz_clip01(phi[xm]) + phc);
+        const double kp = fma(qdk, s0 + fz_sclip(phi[xp]), kmid), km = fma(qdk, fz_sclip(phi[xm]) + s0, kmid);
         adv = (u[xm] * (tm + t0) - u[c] * (t0 + tp)) * (0.5 * idx);
         dif = (kp * (tp - t0) - km * (t0 - tm)) * (idx * idx);
     }
     {   // y
         const double tp = T[yp], tm = T[ym];
-        const double kp = P.k2 + hdk * (phc + fz_clip01(phi[yp])), km = P.k2 + hdk * (fz_clip01(phi[ym]) + phc);
+        const double kp = fma(qdk, s0 + fz_sclip(phi[yp]), kmid), km = fma(qdk, fz_sclip(phi[ym]) + s0, kmid);
         adv += (v[ym] * (tm + t0) - v[c] * (t0 + tp)) * (0.5 * idy);
         dif += (kp * (tp - t0) - km * (t0 - tm)) * (idy * idy);
     }
     {   // z: Dirichlet ghosts 2 T_wall - T, no advective flux through a wall face
         const double tp = z.gp ? 2.0 * P.t_top - t0 : T[zp], tm = z.gm ? 2.0 * P.t_bot - t0 : T[zm];
-        const double kp = P.k2 + hdk * (phc + fz_clip01(phi[zp])), km = P.k2 + hdk * (fz_clip01(phi[zm]) + phc);
+        const double kp = fma(qdk, s0 + fz_sclip(phi[zp]), kmid), km = fma(qdk, fz_sclip(phi[zm]) + s0, kmid);
         const double fp = z.gp ? 0.0 : w[c] * (t0 + tp), fm = z.gm ? 0.0 : w[zm] * (tm + t0);
         adv += (fm - fp) * (0.5 * izf);
         dif += (kp * (tp - t0) * P.idzc[k] - km * (t0 - tm) * P.idzc[k - 1]) * izf;
     }
+    const double phc = 0.5 * s0 + 0.5;
     const double rcp = (P.rho2 + P.drho * phc) * (P.cp2 + (P.cp1 - P.cp2) * phc);
     const double rhs = adv + dif * fz_rcp(rcp);
     Tn[c] = t0 + dt * (gs * rhs + (zs != 0.0 ? zs * hT[c] : 0.0));

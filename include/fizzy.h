@@ -114,11 +114,15 @@ fizzy_status fizzy_set_fields(fizzy_ctx *ctx, const double *u, const double *v, 
  * 3/4; zeta = 0, -17/60, -5/12).  Steps S0-S5 of DESIGN.md: Gamma latch (stage 0), ACDI phi
  * transport, property map, temperature transport (heat on), momentum predictor, Poisson
  * right-hand side + FFT(x,y) + tridiagonal(z) solve, velocity correction and pressure rotation.
+ * After stages 0 and 1 the velocity correction is carried out by the first kernel of the NEXT substep (fused with its
+ * phi transport); any call that reads or replaces a field in between (fizzy_get_fields, fizzy_set_fields,
+ * fizzy_diagnostics, fizzy_stable_dt, fizzy_check_finite, fizzy_poisson_solve) carries it out first, so the state seen
+ * through this interface after a substep is always the corrected one (BASELINE.json:5(v)).
  * FIZZY_EINVAL: stage not in {0,1,2} or dt <= 0.  FIZZY_ESTATE: fields not set / wrong stage. */
 fizzy_status fizzy_rk3_substep(fizzy_ctx *ctx, int stage, double dt);
 
 /* One full RK3 step = the three substeps above in order ("low-storage three-step Runge-Kutta").
- * With fizzy_graph_enable(ctx, 1) the three substeps (about 25 kernel launches) are captured once into a CUDA
+ * With fizzy_graph_enable(ctx, 1) the three substeps (23 kernel launches) are captured once into a CUDA
  * graph per buffer rotation and time step and replayed afterwards -- what matters on the 32^3 .. 128^3
  * configurations, where a substep is launch-bound.  The results are bit-identical to the
  * plain launches.  Graph capture needs a context created on a non-default stream (FIZZY_EINVAL otherwise) and

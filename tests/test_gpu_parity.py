@@ -140,6 +140,23 @@ def test_poisson_solve(fz, oracle_mod, name):
     g.close()
 
 
+@pytest.mark.parametrize("cfg_index,grid", [(1, (32, 16, 4)), (2, (32, 16, 4)), (1, (64, 32, 7)), (4, (32, 32, 6))])
+def test_poisson_solve_shortest_columns(fz, oracle_mod, cfg_index, grid):
+    """The two-sided elimination of the z systems (top half, middle row, bottom half, separator row if z is periodic) on
+    the shortest columns the library accepts (nz = 4: one row per half) and on odd / even nz, periodic and (stretched)
+    walls."""
+    cfg, f, dt, _ = W.make(cfg_index, grid=grid, ndrops=1, radius=0.2)
+    o = oracle_mod.Oracle(cfg)
+    g = fz.Fizzy(cfg)
+    rhs = np.random.default_rng(11).standard_normal(o.shape)
+    po = o.poisson_solve(rhs)
+    pg = np.empty(o.shape)
+    g.fizzy_poisson_solve(np.ascontiguousarray(rhs), pg)
+    g.stream.synchronize()
+    assert field_error(pg, po) <= TOL_SUBSTEP
+    g.close()
+
+
 def test_device_pointers_and_state_errors(fz):
     """set/get with device tensors; stage order and argument errors come back as status codes."""
     import torch

@@ -421,7 +421,7 @@ fizzy_status run_interface(fizzy_ctx *c, bool with_psi)
         FZ_LAUNCHED(FZK_IPSI);
     }
     if (march) {   // marching sweep: nhat and r stay on chip
-        int chunks = 8192 / ((P.nx / ITX) * (P.ny / ITY));
+        int chunks = 4096 / ((P.nx / ITX) * (P.ny / ITY));   // z chunks: about 4096 CTAs (measured: 8192 and 2048 are 0.5-1 % slower at 512^3)
         if (chunks > P.nz / 16) chunks = P.nz / 16;
         if (chunks < 1) chunks = 1;
         const int KC = (P.nz + chunks - 1) / chunks;
@@ -481,7 +481,7 @@ cudaError_t launch_momentum3(fizzy_ctx *c, dim3 grid, dim3 block, const FzMomArg
     const FzMomArgs &A = *Ap;
     if (P.nx >= MTX && P.ny >= MTY) {   // 2.5-D marching kernel
         const int tiles = (P.nx / MTX) * (P.ny / MTY);
-        int chunks = 8192 / tiles;
+        int chunks = 4096 / tiles;
         if (chunks > P.nz / 16) chunks = P.nz / 16;
         if (chunks < 1) chunks = 1;
         const int KC = (P.nz + chunks - 1) / chunks;

@@ -48,13 +48,14 @@ __device__ __forceinline__ double fz_sharp2(double ra, double rb)
     return s * t * t;
 }
 
-// r = sqrt(q), q = (phic + delta)/(1 - phic + delta) (N2); 1 - phic + delta in [delta, 1 + delta], q in
-// [delta, 1/delta] with delta >= 1e-150 (fizzy_create): all normal, so the branch-free helpers apply
+// r = sqrt(q), q = a/b, a = phic + delta, b = 1 - phic + delta (N2), as a * rsqrt(a b): ONE rsqrt and no reciprocal.
+// a b lies in [delta (1 + delta), (1/2 + delta)^2] with delta >= 1e-150 (fizzy_create): normal, so the branch-free
+// helper applies
 __device__ __forceinline__ double fz_sqrtq(double phi, double delta)
 {
     const double ph = fz_clip01(phi);
-    const double q = (ph + delta) * fz_rcp(1.0 - ph + delta);
-    return q * fz_rsqrt(q);
+    const double a = ph + delta, b = 1.0 - ph + delta;
+    return a * fz_rsqrt(a * b);
 }
 
 template <bool STORE_R>

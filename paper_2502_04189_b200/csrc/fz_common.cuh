@@ -90,6 +90,14 @@ __device__ __forceinline__ double fz_rsqrt(double a)
 }
 // reciprocal of a normal, finite d of EITHER sign whose reciprocal is normal (tridiagonal pivots)
 __device__ __forceinline__ double fz_rcp_signed(double d) { return fz_rcp(d); }   // the seed keeps the sign
+// psi = eps ln q of a phase field value, q = (phic + delta)/(1 - phic + delta) (N2); 1 - phic + delta lies in
+// [delta, 1 + delta], delta >= 1e-150: the branch-free reciprocal applies
+__device__ __forceinline__ double fz_psi(const FzP &P, double f)
+{
+    const double ph = fz_clip01(f);
+    return P.eps * log((ph + P.delta) * fz_rcp(1.0 - ph + P.delta));
+}
+
 // prefetch the 128-byte line at p into L2 (no register, no scoreboard)
 __device__ __forceinline__ void fz_prefetch_l2(const void *p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
 

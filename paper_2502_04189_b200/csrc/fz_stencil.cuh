@@ -44,9 +44,8 @@ __global__ void k_iface_psi(FzP P, const double *__restrict__ phi, double *__res
     FZ_CELL_IJK
     const long long c = i + (long long)P.nx * (j + (long long)P.ny * k);
     const double ph = fz_clip01(phi[c]);
-    const double q = (ph + P.delta) / (1.0 - ph + P.delta);
-    psi[c] = P.eps * log(q);
-    rr[c] = sqrt(q);
+    psi[c] = fz_psi(P, phi[c]);
+    rr[c] = sqrt((ph + P.delta) / (1.0 - ph + P.delta));
 }
 
 // (b) nhat = G / max(|G|, 1e-30), G = central difference of psi (mirror at walls)
@@ -131,11 +130,11 @@ __global__ void k_phi_update(FzP P, const double *__restrict__ phi, const double
 {
     FZ_CELL_IJK
     const FzZ z = fz_zn(P, k);
-    const long long pl = (long long)P.ny * k;
-    const long long c = i + P.nx * (j + pl);
-    const long long xp = fz_ip(i, P.nx) + P.nx * (j + pl), xm = fz_im(i, P.nx) + P.nx * (j + pl);
-    const long long yp = i + P.nx * (fz_ip(j, P.ny) + pl), ym = i + P.nx * (fz_im(j, P.ny) + pl);
-    const long long zp = c + (long long)(z.kp - k) * P.sxy, zm = c + (long long)(z.km - k) * P.sxy;
+    const unsigned nx = P.nx, sxy = (unsigned)P.sxy;   // 32-bit offsets: N < 2^31 (fizzy_create)
+    const unsigned pl = (unsigned)k * sxy, row = pl + nx * j, c = row + i;
+    const unsigned xp = row + fz_ip(i, P.nx), xm = row + fz_im(i, P.nx);
+    const unsigned yp = pl + nx * fz_ip(j, P.ny) + i, ym = pl + nx * fz_im(j, P.ny) + i;
+    const unsigned zp = (unsigned)z.kp * sxy + nx * j + i, zm = (unsigned)z.km * sxy + nx * j + i;
     const double f0 = phi[c];
     const double Fxp = -u[c] * 0.5 * (f0 + phi[xp]), Fxm = -u[xm] * 0.5 * (phi[xm] + f0);
     const double Fyp = -v[c] * 0.5 * (f0 + phi[yp]), Fym = -v[ym] * 0.5 * (phi[ym] + f0);
@@ -146,10 +145,7 @@ __global__ void k_phi_update(FzP P, const double *__restrict__ phi, const double
     const double fn = f0 + dt * (gs * rhs + (zs != 0.0 ? zs * hphi[c] : 0.0));
     phin[c] = fn;
     if (keep_h) hphi[c] = rhs;   // not at stage 2: the next stage has zeta = 0 and never reads it
-    // psi of phi_new for the interface sweep (same formula as k_iface_psi)
-    const double ph = fz_clip01(fn);
-    const double q = (ph + P.delta) / (1.0 - ph + P.delta);
-    psi[c] = P.eps * log(q);
+    psi[c] = fz_psi(P, fn);
 }
 
 // ---------------------------------------------------------------- S5 of the previous substep fused with S1
@@ -203,9 +199,7 @@ __global__ void k_corr_phi(FzP P, const double *__restrict__ us, const double *_
     const double fn = f0 + dt * (gs * rhs + (zs != 0.0 ? zs * hphi[c] : 0.0));
     phin[c] = fn;
     if (keep_h) hphi[c] = rhs;
-    const double ph = fz_clip01(fn);
-    const double q = (ph + P.delta) / (1.0 - ph + P.delta);
-    psi[c] = P.eps * log(q);
+    psi[c] = fz_psi(P, fn);
 }
 
 // ---------------------------------------------------------------- S2b: temperature transport (N14)
@@ -267,14 +261,14 @@ __global__ void k_correct(FzP P, const double *__restrict__ us, const double *__
 {
     FZ_CELL_IJK
     const FzZ z = fz_zn(P, k);
-    const long long pl = (long long)P.ny * k;
-    const long long c = i + P.nx * (j + pl);
+    const unsigned nx = P.nx, sxy = (unsigned)P.sxy;   // 32-bit offsets: N < 2^31 (fizzy_create)
+    const unsigned pl = (unsigned)k * sxy, c = pl + nx * j + i;
     const double p0 = pn[c];
     if (phat) phat[c] = 2.0 * p0 - pold[c];
-    const double un = fz_corr(us[c], coef, pn[fz_ip(i, P.nx) + P.nx * (j + pl)], p0, P.idx);
-    const double vn = fz_corr(vs[c], coef, pn[i + P.nx * (fz_ip(j, P.ny) + pl)], p0, P.idy);
+    const double un = fz_corr(us[c], coef, pn[pl + nx * j + fz_ip(i, P.nx)], p0, P.idx);
+    const double vn = fz_corr(vs[c], coef, pn[pl + nx * fz_ip(j, P.ny) + i], p0, P.idy);
     double wn = 0.0;
-    if (k < P.kzf) wn = fz_corr(ws[c], coef, pn[c + (long long)(z.kp - k) * P.sxy], p0, P.idzc[k]);
+    if (k < P.kzf) wn = fz_corr(ws[c], coef, pn[(unsigned)z.kp * sxy + nx * j + i], p0, P.idzc[k]);
     u[c] = un;
     v[c] = vn;
     w[c] = wn;

@@ -204,8 +204,10 @@ __global__ void k_corr_phi(FzP P, const double *__restrict__ us, const double *_
 
 // ---------------------------------------------------------------- S2b: temperature transport (N14)
 // RHS_T = D(-u_a Tbar_a) + D(kbar_a d_a T)/(rho cp), properties from phi_new;  k is linear in clip(phi),
-// so kbar_a = k2 + (k1-k2) * 0.5 (phic + phic(+1_a)).  32-bit offsets (N < 2^31), 8 CTAs/SM.
-__global__ void __launch_bounds__(256, 6)
+// so kbar_a = k2 + (k1-k2) * 0.5 (phic + phic(+1_a)).  32-bit offsets (N < 2^31).  64 registers, four CTAs per SM: all 21
+// loads of a thread in flight at once (at 40 registers / six CTAs the kernel waited on serialised loads: 0.52 -> 0.44 ms at
+// 512x256x256).
+__global__ void __launch_bounds__(256, 4)
 k_temp_update(FzP P, const double *__restrict__ T, const double *__restrict__ phi,
               const double *__restrict__ u, const double *__restrict__ v,
               const double *__restrict__ w, double *__restrict__ hT,

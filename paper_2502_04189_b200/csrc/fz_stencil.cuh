@@ -122,7 +122,8 @@ __global__ void k_iface_flux(FzP P, const double *__restrict__ phi, const double
 // ---------------------------------------------------------------- S1: ACDI phi transport
 // RHSphi = D(-u_a phibar_a) + Gamma D(Rn);  phi <- phi + dt (g RHS + z RHS_old)   (BASELINE.json:5(i))
 // also writes psi = eps ln q of phi_new (N2), the input of k_iface_march (r = sqrt q is recomputed there)
-__global__ void k_phi_update(FzP P, const double *__restrict__ phi, const double *__restrict__ u,
+__global__ void __launch_bounds__(256, 5)
+k_phi_update(FzP P, const double *__restrict__ phi, const double *__restrict__ u,
                              const double *__restrict__ v, const double *__restrict__ w,
                              const double *__restrict__ divrn, double *__restrict__ hphi,
                              double *__restrict__ phin, double *__restrict__ psi,
@@ -161,7 +162,8 @@ __device__ __forceinline__ double fz_corr(double us, double coef, double p_hi, d
 // the corrected velocity is written but never read back by S1: -24 B/cell against k_correct + k_phi_update.
 // (After stage 2 k_correct runs on its own: Gamma of the next step needs max|u| before its S1, N15.)
 // phat != NULL (rho1 != rho2): also p_hat = 2 p_new - p_old (N7).
-__global__ void k_corr_phi(FzP P, const double *__restrict__ us, const double *__restrict__ vs,
+__global__ void __launch_bounds__(256, 5)
+k_corr_phi(FzP P, const double *__restrict__ us, const double *__restrict__ vs,
                            const double *__restrict__ ws, const double *__restrict__ pn,
                            const double *__restrict__ pold, double *__restrict__ phat,
                            double *__restrict__ u, double *__restrict__ v, double *__restrict__ w,

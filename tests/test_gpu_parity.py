@@ -157,6 +157,49 @@ def test_poisson_solve_shortest_columns(fz, oracle_mod, cfg_index, grid):
     g.close()
 
 
+# odd and prime nz, nz barely above the tile / chunk sizes, nx != ny, every config's physics: one whole step each
+ODD_SHAPES = [(0, (32, 32, 33)), (0, (64, 64, 7)), (1, (32, 32, 20)), (1, (64, 32, 37)), (2, (32, 64, 24)),
+              (2, (64, 32, 17)), (3, (32, 16, 19)), (3, (64, 64, 41)), (4, (32, 32, 28)), (4, (64, 16, 23))]
+
+
+@pytest.mark.parametrize("index,grid", ODD_SHAPES)
+def test_full_step_odd_shapes(fz, oracle_mod, index, grid):
+    """A whole RK3 step (deferred-correction path) on grids whose nz is odd, prime or just past a chunk boundary of the
+    marching kernels and of the two-sided z sweeps (unequal halves), for the physics of all five configs."""
+    cfg, f, dt, _ = W.make(index, grid=grid, ndrops=1, radius=0.2 if index else None)
+    o = oracle_mod.Oracle(cfg)
+    o.set_fields(**f)
+    g = fz.Fizzy(cfg)
+    g.set_fields_numpy(**f)
+    o.step(dt)
+    g.step(dt)
+    fo, fg = o.get_fields(), g.get_fields_numpy()
+    for k in fo:
+        assert np.isfinite(fg[k]).all(), (grid, k)
+        assert field_error(fg[k], fo[k]) <= TOL_SUBSTEP, (index, grid, k, field_error(fg[k], fo[k]))
+    g.close()
+    o.close()
+
+
+@pytest.mark.parametrize("n", [8, 16, 32, 64, 128, 256, 512])
+def test_poisson_solve_every_transform_length(fz, oracle_mod, n):
+    """Every instantiated line length of the x transforms (r2c with the fused right-hand side path off; c2r with the TMA box
+    loads: 1 to 3 boxes, 64- and 128-byte rows) and of the fused y transform / z sweeps (G = 1 and G = 4 groups), each once as
+    nx and once as ny, periodic and wall z (1024 is in CASES)."""
+    for grid, ci in (((n, 16, 6), 1), ((16, n, 5), 2)):
+        cfg, f, dt, _ = W.make(ci, grid=grid, ndrops=1, radius=0.2)
+        o = oracle_mod.Oracle(cfg)
+        g = fz.Fizzy(cfg)
+        rhs = np.random.default_rng(n).standard_normal(o.shape)
+        po = o.poisson_solve(rhs)
+        pg = np.empty(o.shape)
+        g.fizzy_poisson_solve(np.ascontiguousarray(rhs), pg)
+        g.stream.synchronize()
+        assert field_error(pg, po) <= TOL_SUBSTEP, (grid, field_error(pg, po))
+        g.close()
+        o.close()
+
+
 def test_device_pointers_and_state_errors(fz):
     """set/get with device tensors; stage order and argument errors come back as status codes."""
     import torch

@@ -197,6 +197,26 @@ cudaEvent_t take_event(fizzy_ctx *c)
 
 cudaError_t launch_momentum(fizzy_ctx *c, dim3 grid, dim3 block, const FzMomArgs *A);   // defined with the substep
 
+// Planes per z chunk of a marching kernel: a CTA marches KC planes after `ov` planes of pipeline fill, `slots` CTAs run at
+// a time.  Cost model: (waves, at least one, + half a wave of tail) x (KC + ov); ties go to the longer chunk.  Large grids
+// get 64-128 planes per chunk (measured at 512^3: 4096-8192 CTAs are the flat optimum), small ones short chunks, so
+// that a 32^3 grid is not marched by eight CTAs of nineteen plane steps each.
+int march_chunk(int nz, int tiles, int slots, int ov)
+{
+    int best = nz;
+    double best_cost = 1e300;
+    for (int kc = 4; ; kc *= 2) {
+        if (kc > nz) kc = nz;
+        const double ctas = (double)tiles * ((nz + kc - 1) / kc);
+        double waves = ctas / slots + 0.5;
+        if (waves < 1.0) waves = 1.0;
+        const double cost = waves * (kc + ov);
+        if (cost <= best_cost * 1.0000001) { best_cost = cost; best = kc; }
+        if (kc == nz) break;
+    }
+    return best;
+}
+
 void cell_launch(const fizzy_ctx *c, dim3 &grid, dim3 &block)
 {
     const int bx = c->P.nx < 64 ? c->P.nx : 64;
@@ -421,10 +441,7 @@ fizzy_status run_interface(fizzy_ctx *c, bool with_psi)
         FZ_LAUNCHED(FZK_IPSI);
     }
     if (march) {   // marching sweep: nhat and r stay on chip
-        int chunks = 4096 / ((P.nx / ITX) * (P.ny / ITY));   // z chunks: about 4096 CTAs (measured: 8192 and 2048 are 0.5-1 % slower at 512^3)
-        if (chunks > P.nz / 16) chunks = P.nz / 16;
-        if (chunks < 1) chunks = 1;
-        const int KC = (P.nz + chunks - 1) / chunks;
+        const int KC = march_chunk(P.nz, (P.nx / ITX) * (P.ny / ITY), 148 * 2, 4);
         const dim3 g(P.nx / ITX, P.ny / ITY, (P.nz + KC - 1) / KC);
         FZ_TB(FZK_IMARCH);
         if (c->varrho)
@@ -481,10 +498,7 @@ cudaError_t launch_momentum3(fizzy_ctx *c, dim3 grid, dim3 block, const FzMomArg
     const FzMomArgs &A = *Ap;
     if (P.nx >= MTX && P.ny >= MTY) {   // 2.5-D marching kernel
         const int tiles = (P.nx / MTX) * (P.ny / MTY);
-        int chunks = 4096 / tiles;
-        if (chunks > P.nz / 16) chunks = P.nz / 16;
-        if (chunks < 1) chunks = 1;
-        const int KC = (P.nz + chunks - 1) / chunks;
+        const int KC = march_chunk(P.nz, tiles, 148 * FzMomFields<VR, HT>::MINB, 3);
         const dim3 g(P.nx / MTX, P.ny / MTY, (P.nz + KC - 1) / KC);
         k_momentum_march<VR, VM, HT><<<g, dim3(MTX, MTY), smem, c->stream>>>(P, A, KC);
     } else {                            // tiny grids: one thread per cell straight from global memory

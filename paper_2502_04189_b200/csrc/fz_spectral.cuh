@@ -137,15 +137,20 @@ __global__ void k_tri_tables(FzP P, FzTri Tt)
 // G = 1 at ny = 512: there four single-transform CTAs share an SM (56 KB of shared memory each at most).
 #define SPEC_FL 5    // forward, lines per group: one fixed scratch line + a ring of SPEC_FL-1 (current | SPEC_FL-2 in flight)
 #define SPEC_FLB 4   // backward: scratch + ring of 3 lines (current | 2 in flight) and a ring of 2 rows of INV (E)
-__host__ __device__ constexpr int spec_groups(int log2n) { return log2n == 8 ? 4 : 1; }
+__host__ __device__ constexpr int spec_groups(int log2n) { return log2n <= 8 ? 4 : 1; }
 __host__ __device__ constexpr int spec_minb(int log2n) { return log2n == 9 ? 4 : (log2n >= 8 ? 2 : 1); }
+// Short lines (ny < 256: fewer than 32 threads per transform): a group is still one whole warp and transforms
+// MPG = 32/(ny/8) x-modes side by side, so that the named barriers see whole warps and a 128^3 grid is not solved by 130
+// half-warps.  GT = threads per group.
+__host__ __device__ constexpr int spec_mpg(int log2n) { return log2n >= 8 ? 1 : 32 / ((1 << log2n) / 8); }
+__host__ __device__ constexpr int spec_gt(int log2n) { return log2n >= 8 ? (1 << log2n) / 8 : 32; }
 
 __host__ __device__ inline size_t fz_spec_smem(int log2n, bool fwd, bool cyclic)
 {
-    const int n = 1 << log2n, nt = n / 8, G = spec_groups(log2n);
+    const int n = 1 << log2n, G = spec_groups(log2n), MPG = spec_mpg(log2n), GT = spec_gt(log2n);
     const size_t state = G > 1 ? 1 : 0;   // the handoff buffers exist only when there is somebody to hand over to
-    if (fwd) return (size_t)G * SPEC_FL * SPEC_LINE(n) * 16 + state * nt * 8 * (cyclic ? 48 : 24);
-    return (size_t)G * SPEC_FLB * SPEC_LINE(n) * 16 + (size_t)G * 2 * n * 8 * (cyclic ? 2 : 1) + state * nt * 8 * 16 + 16;
+    if (fwd) return (size_t)G * MPG * SPEC_FL * SPEC_LINE(n) * 16 + state * GT * 8 * (cyclic ? 48 : 24);
+    return (size_t)G * MPG * SPEC_FLB * SPEC_LINE(n) * 16 + (size_t)G * MPG * 2 * n * 8 * (cyclic ? 2 : 1) + state * GT * 8 * 16 + 16;
 }
 
 __device__ __forceinline__ void fz_bar_sync(int id, int n) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(n) : "memory"); }
@@ -156,30 +161,33 @@ __device__ __forceinline__ void fz_bar_arrive(int id, int n) { asm volatile("bar
 // tail step (the top half: row mid; the bottom half of a cyclic system: row nz-1) only transforms its plane and
 // forms the half's contribution to r1 (and r2) in SIDE.
 template <bool CYCLIC, int LOG2N, int G>
-__global__ void __launch_bounds__(G * ((1 << LOG2N) / 8), spec_minb(LOG2N))
+__global__ void __launch_bounds__(G * spec_gt(LOG2N), spec_minb(LOG2N))
 k_spec_fwd(FzP P, FzTri Tt, double2 *__restrict__ spec, const double2 *__restrict__ tw)
 {
     extern __shared__ __align__(16) double2 sms[];
-    constexpr int n = 1 << LOG2N, nt = n / 8, LN = SPEC_LINE(n);
-    const int jt = threadIdx.x, g = threadIdx.y, nz = P.nz, half = blockIdx.y;
-    double2 *scratch = sms + g * SPEC_FL * LN, *lines = scratch + LN;   // ring of RL = SPEC_FL-1 lines
-    double2 *st_dp = sms + G * SPEC_FL * LN;                              // [q][jt]
-    double *st_hp = reinterpret_cast<double *>(st_dp + 8 * nt);
-    double2 *st_h = reinterpret_cast<double2 *>(st_hp + 8 * nt);   // cyclic only
-    double *st_f = reinterpret_cast<double *>(st_h + 8 * nt);
+    constexpr int n = 1 << LOG2N, nt = n / 8, LN = SPEC_LINE(n), MPG = spec_mpg(LOG2N), GT = spec_gt(LOG2N), SL = MPG * LN;
+    const int tx = threadIdx.x, jt = tx & (nt - 1), ms = tx / nt, g = threadIdx.y, nz = P.nz, half = blockIdx.y;
+    // x-mode of this thread; a CTA past the last mode repeats it without storing (its threads still meet the barriers)
+    const bool live = (int)blockIdx.x * MPG + ms < P.nxh;
+    const int l = live ? (int)blockIdx.x * MPG + ms : P.nxh - 1;
+    double2 *scratch = sms + (g * SPEC_FL * MPG + ms) * LN, *lines = scratch + SL;   // ring of RL = SPEC_FL-1 slots of MPG lines
+    double2 *st_dp = sms + G * SPEC_FL * SL;                                          // [q][tx]
+    double *st_hp = reinterpret_cast<double *>(st_dp + 8 * GT);
+    double2 *st_h = reinterpret_cast<double2 *>(st_hp + 8 * GT);   // cyclic only
+    double *st_f = reinterpret_cast<double *>(st_h + 8 * GT);
     FzLineFFT<LOG2N, -1> fft;
     fft.init(tw, jt);
-    if (G > 1) { fft.bar_id = 1 + G + g; fft.bar_n = nt; }
+    if (G > 1) { fft.bar_id = 1 + G + g; fft.bar_n = GT; }
     const FzHalf H = fz_tri_half(Tt, nz, half);
     const int mid = fz_tri_mid(nz);
     const bool has_tail = CYCLIC || half == 0;
     const int NS = H.S + (has_tail ? 1 : 0), ktail = half == 0 ? mid : nz - 1;
-    const long long M = (long long)P.nxh * n, base = (long long)blockIdx.x * n;
+    const long long M = (long long)P.nxh * n, base = (long long)l * n;
     auto issue = [&](int s, int slot) {
         if (s < NS) {
             const int k = s < H.S ? H.kfirst + H.dk * s : ktail;
             const double2 *gp = spec + (long long)k * M + base;
-            double2 *d = lines + slot * LN;
+            double2 *d = lines + slot * SL;
 #pragma unroll
             for (int q = 0; q < 8; ++q) { const int i = jt + q * nt; fz_cp_async16(d + SPEC_PADI(i), gp + i); }
         }
@@ -188,7 +196,7 @@ k_spec_fwd(FzP P, FzTri Tt, double2 *__restrict__ spec, const double2 *__restric
     for (int d = 0; d < SPEC_FL - 2; ++d) { issue(g + d * G, d); fz_cp_async_commit(); }
     double lam[8];
     const double f0 = H.HI[nz - 1], lom = H.LO[mid];
-    const double lamx = Tt.lamx[blockIdx.x];
+    const double lamx = Tt.lamx[l];
 #pragma unroll
     for (int q = 0; q < 8; ++q) lam[q] = lamx + Tt.lamy[jt + q * nt];
     double2 dp[8], h[8];
@@ -203,17 +211,17 @@ k_spec_fwd(FzP P, FzTri Tt, double2 *__restrict__ spec, const double2 *__restric
         issue(s + (SPEC_FL - 2) * G, tgt);
         fz_cp_async_commit();
         double2 v[8];
-        fft.smem_to_regs(jt, lines + cur * LN, scratch, v);
+        fft.smem_to_regs(jt, lines + cur * SL, scratch, v);
         // the recurrence state of step s-1 (token from its group)
         if (s == 0) {
 #pragma unroll
             for (int q = 0; q < 8; ++q) { dp[q] = make_double2(0, 0); h[q] = make_double2(0, 0); f[q] = f0; hp[q] = 0.0; }
         } else if (G > 1) {
-            fz_bar_sync(1 + g, 2 * nt);
+            fz_bar_sync(1 + g, 2 * GT);
 #pragma unroll
             for (int q = 0; q < 8; ++q) {
-                dp[q] = st_dp[q * nt + jt]; hp[q] = st_hp[q * nt + jt];
-                if (CYCLIC) { h[q] = st_h[q * nt + jt]; f[q] = st_f[q * nt + jt]; }
+                dp[q] = st_dp[q * GT + tx]; hp[q] = st_hp[q * GT + tx];
+                if (CYCLIC) { h[q] = st_h[q * GT + tx]; f[q] = st_f[q * GT + tx]; }
             }
         }
         if (s < H.S) {
@@ -221,7 +229,7 @@ k_spec_fwd(FzP P, FzTri Tt, double2 *__restrict__ spec, const double2 *__restric
             double2 *out = spec + (long long)k * M + base;
             const double lo = H.LO[k], hi = H.HI[k];
             // N17: x_{nz-1} = 0 for the singular mode (walls): first row of the bottom half; its thread is (l, m) = (0, 0), q = 0
-            const bool sing = !CYCLIC && half == 1 && s == 0 && blockIdx.x == 0 && jt == 0;
+            const bool sing = !CYCLIC && half == 1 && s == 0 && l == 0 && jt == 0;
 #pragma unroll
             for (int q = 0; q < 8; ++q) {
                 double inv = fz_rcp_signed(fz_tri_den(lo, hi, lam[q], hp[q]));
@@ -238,19 +246,21 @@ k_spec_fwd(FzP P, FzTri Tt, double2 *__restrict__ spec, const double2 *__restric
             if (G > 1 && s < NS - 1) {   // hand the state to the group of step s+1
 #pragma unroll
                 for (int q = 0; q < 8; ++q) {
-                    st_dp[q * nt + jt] = dp[q]; st_hp[q * nt + jt] = hp[q];
-                    if (CYCLIC) { st_h[q * nt + jt] = h[q]; st_f[q * nt + jt] = f[q]; }
+                    st_dp[q * GT + tx] = dp[q]; st_hp[q * GT + tx] = hp[q];
+                    if (CYCLIC) { st_h[q * GT + tx] = h[q]; st_f[q * GT + tx] = f[q]; }
                 }
-                fz_bar_arrive(1 + (g + 1 == G ? 0 : g + 1), 2 * nt);
+                fz_bar_arrive(1 + (g + 1 == G ? 0 : g + 1), 2 * GT);
             }
+            if (live) {
 #pragma unroll
-            for (int q = 0; q < 8; ++q) out[jt + q * nt] = dp[q];
-            if (!has_tail && s == H.S - 1) {   // bottom half, walls: r1 contribution -c_mid d'_bot
+                for (int q = 0; q < 8; ++q) out[jt + q * nt] = dp[q];
+            }
+            if (live && !has_tail && s == H.S - 1) {   // bottom half, walls: r1 contribution -c_mid d'_bot
                 double2 *sd = Tt.side + 2 * M + base;
 #pragma unroll
                 for (int q = 0; q < 8; ++q) sd[jt + q * nt] = make_double2(-lom * dp[q].x, -lom * dp[q].y);
             }
-        } else {   // tail: v = transformed row mid (top) / row nz-1 (bottom, cyclic)
+        } else if (live) {   // tail: v = transformed row mid (top) / row nz-1 (bottom, cyclic)
             double2 *s1 = Tt.side + (half == 0 ? 0 : 2 * M) + base, *s2 = s1 + M;
 #pragma unroll
             for (int q = 0; q < 8; ++q) {
@@ -275,26 +285,29 @@ k_spec_fwd(FzP P, FzTri Tt, double2 *__restrict__ spec, const double2 *__restric
 // plane to load).  scal[2] / scal[6] receive the halves' parts of the dzf-weighted mean of mode (0,0) (gauge, N17),
 // accumulated in plane order under the token.
 template <bool CYCLIC, int LOG2N, int G>
-__global__ void __launch_bounds__(G * ((1 << LOG2N) / 8), spec_minb(LOG2N))
+__global__ void __launch_bounds__(G * spec_gt(LOG2N), spec_minb(LOG2N))
 k_spec_bwd(FzP P, FzTri Tt, double2 *__restrict__ spec, const double2 *__restrict__ tw,
            double *__restrict__ scal)
 {
     extern __shared__ __align__(16) double2 sms[];
     constexpr int n = 1 << LOG2N, nt = n / 8, LN = SPEC_LINE(n), NT = CYCLIC ? 2 : 1;
+    constexpr int MPG = spec_mpg(LOG2N), GT = spec_gt(LOG2N), SL = MPG * LN, SR = MPG * n * NT;
     constexpr int RL = SPEC_FLB - 1;                                    // ring of lines: current + 2 in flight
-    const int jt = threadIdx.x, g = threadIdx.y, nz = P.nz, half = blockIdx.y;
-    double2 *scratch = sms + g * SPEC_FLB * LN, *lines = scratch + LN;
-    double *rows0 = reinterpret_cast<double *>(sms + G * SPEC_FLB * LN);
-    double *rows = rows0 + g * 2 * n * NT;                              // [slot: current | next][INV | E][n]
-    double2 *st_x = reinterpret_cast<double2 *>(rows0 + G * 2 * n * NT);   // [q][jt]
-    double *st_acc = reinterpret_cast<double *>(st_x + (G > 1 ? 8 * nt : 0));   // G = 1: no handoff buffer
+    const int tx = threadIdx.x, jt = tx & (nt - 1), ms = tx / nt, g = threadIdx.y, nz = P.nz, half = blockIdx.y;
+    const bool live = (int)blockIdx.x * MPG + ms < P.nxh;               // see k_spec_fwd
+    const int l = live ? (int)blockIdx.x * MPG + ms : P.nxh - 1;
+    double2 *scratch = sms + (g * SPEC_FLB * MPG + ms) * LN, *lines = scratch + SL;
+    double *rows0 = reinterpret_cast<double *>(sms + G * SPEC_FLB * SL);
+    double *rows = rows0 + (g * 2 * MPG + ms) * n * NT;                 // [slot: current | next][mode][INV | E][n]
+    double2 *st_x = reinterpret_cast<double2 *>(rows0 + G * 2 * SR);    // [q][tx]
+    double *st_acc = reinterpret_cast<double *>(st_x + (G > 1 ? 8 * GT : 0));   // G = 1: no handoff buffer
     FzLineFFT<LOG2N, +1> fft;
     fft.init(tw, jt);
-    if (G > 1) { fft.bar_id = 1 + G + g; fft.bar_n = nt; }
+    if (G > 1) { fft.bar_id = 1 + G + g; fft.bar_n = GT; }
     const FzHalf H = fz_tri_half(Tt, nz, half);
     const int mid = fz_tri_mid(nz);
     const int NSTEP = half == 0 ? mid + 1 : H.S + (CYCLIC ? 1 : 0);
-    const long long M = (long long)P.nxh * n, base = (long long)blockIdx.x * n;
+    const long long M = (long long)P.nxh * n, base = (long long)l * n;
     // step t: a row with a plane to load (regular), or x_mid / X (special)
     auto special = [&](int t) { return half == 0 ? t == 0 : t == H.S; };
     auto plane = [&](int t) { return half == 0 ? mid - t : (t < H.S ? mid + 1 + t : nz - 1); };
@@ -303,7 +316,7 @@ k_spec_bwd(FzP P, FzTri Tt, double2 *__restrict__ spec, const double2 *__restric
             const int k = plane(t);
             const double *gi = Tt.inv + (long long)k * M + base;
             const double *ge = Tt.e + (long long)k * M + base;
-            double *dr = rows + rslot * n * NT;
+            double *dr = rows + rslot * SR;
 #pragma unroll
             for (int q = 0; q < 4; ++q) {
                 const int i = 2 * (jt + q * nt);
@@ -315,7 +328,7 @@ k_spec_bwd(FzP P, FzTri Tt, double2 *__restrict__ spec, const double2 *__restric
     auto issue_line = [&](int t, int slot) {
         if (t < NSTEP && !special(t)) {
             const double2 *gp = spec + (long long)plane(t) * M + base;
-            double2 *d = lines + slot * LN;
+            double2 *d = lines + slot * SL;
 #pragma unroll
             for (int q = 0; q < 8; ++q) { const int i = jt + q * nt; fz_cp_async16(d + SPEC_PADI(i), gp + i); }
         }
@@ -343,7 +356,7 @@ k_spec_bwd(FzP P, FzTri Tt, double2 *__restrict__ spec, const double2 *__restric
             X[q] = make_double2(0, 0);
         }
     }
-    const bool gauge = blockIdx.x == 0 && jt == 0;   // owner of mode (l, m) = (0, 0)
+    const bool gauge = l == 0 && jt == 0;   // owner of mode (l, m) = (0, 0)
     int cur = 0, rcur = 0;
     for (int t = g; t < NSTEP; t += G) {
         const int nxt = cur + 1 == RL ? 0 : cur + 1, tgt = cur == 0 ? RL - 1 : cur - 1;
@@ -353,12 +366,12 @@ k_spec_bwd(FzP P, FzTri Tt, double2 *__restrict__ spec, const double2 *__restric
         fz_cp_async_commit();
         issue_line(t + 2 * G, tgt);
         fz_cp_async_commit();
-        double2 *ln = lines + cur * LN;
-        const double *iv = rows + rcur * n * NT, *ev = iv + n;
+        double2 *ln = lines + cur * SL;
+        const double *iv = rows + rcur * SR, *ev = iv + n;
         if (G > 1 && t > 0) {   // the previous x from the group of step t-1
-            fz_bar_sync(1 + g, 2 * nt);
+            fz_bar_sync(1 + g, 2 * GT);
 #pragma unroll
-            for (int q = 0; q < 8; ++q) xn[q] = st_x[q * nt + jt];
+            for (int q = 0; q < 8; ++q) xn[q] = st_x[q * GT + tx];
         }
         const int k = plane(t);
         if (!special(t)) {
@@ -388,16 +401,18 @@ k_spec_bwd(FzP P, FzTri Tt, double2 *__restrict__ spec, const double2 *__restric
         }
         if (G > 1 && t < NSTEP - 1) {
 #pragma unroll
-            for (int q = 0; q < 8; ++q) st_x[q * nt + jt] = xn[q];
-            fz_bar_arrive(1 + (g + 1 == G ? 0 : g + 1), 2 * nt);
+            for (int q = 0; q < 8; ++q) st_x[q * GT + tx] = xn[q];
+            fz_bar_arrive(1 + (g + 1 == G ? 0 : g + 1), 2 * GT);
         }
         double2 v[8];
 #pragma unroll
         for (int q = 0; q < 8; ++q) v[q] = xn[q];
         const double2 *res = fft.regs_to_smem(jt, ln, scratch, v);
         double2 *out = spec + (long long)k * M + base;
+        if (live) {
 #pragma unroll
-        for (int q = 0; q < 8; ++q) { const int m = jt + q * nt; out[m] = res[SPEC_PADI(m)]; }
+            for (int q = 0; q < 8; ++q) { const int m = jt + q * nt; out[m] = res[SPEC_PADI(m)]; }
+        }
         cur = nxt;
         rcur ^= 1;
     }
@@ -410,15 +425,15 @@ template <bool CYCLIC, int LOG2N>
 cudaError_t fz_spec_launch_one(int which, const FzP &P, const FzTri &Tt, double2 *spec, const double2 *tw,
                                double *scal, cudaStream_t st)
 {
-    constexpr int n = 1 << LOG2N, GF = spec_groups(LOG2N), GB = spec_groups(LOG2N);
+    constexpr int GF = spec_groups(LOG2N), GB = spec_groups(LOG2N), MPG = spec_mpg(LOG2N);
     const size_t sf = fz_spec_smem(LOG2N, true, CYCLIC), sb = fz_spec_smem(LOG2N, false, CYCLIC);
     if (which < 0) {
         cudaError_t e = cudaFuncSetAttribute(k_spec_fwd<CYCLIC, LOG2N, GF>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sf);
         if (e == cudaSuccess) e = cudaFuncSetAttribute(k_spec_bwd<CYCLIC, LOG2N, GB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sb);
         return e;
     }
-    if (which == 0) k_spec_fwd<CYCLIC, LOG2N, GF><<<dim3(P.nxh, 2), dim3(n / 8, GF), sf, st>>>(P, Tt, spec, tw);
-    else k_spec_bwd<CYCLIC, LOG2N, GB><<<dim3(P.nxh, 2), dim3(n / 8, GB), sb, st>>>(P, Tt, spec, tw, scal);
+    if (which == 0) k_spec_fwd<CYCLIC, LOG2N, GF><<<dim3((P.nxh + MPG - 1) / MPG, 2), dim3(spec_gt(LOG2N), GF), sf, st>>>(P, Tt, spec, tw);
+    else k_spec_bwd<CYCLIC, LOG2N, GB><<<dim3((P.nxh + MPG - 1) / MPG, 2), dim3(spec_gt(LOG2N), GB), sb, st>>>(P, Tt, spec, tw, scal);
     return cudaSuccess;
 }
 

@@ -257,6 +257,37 @@ def graph_compare(torch, Fizzy, device):
     return out
 
 
+def varcoef_bench(args):
+    """SURVEY.md 8(f)-4 (not part of the RK3 step): fizzy_poisson_solve_varcoef on the phase field of the chosen workload,
+    random right-hand side, to a relative residual of 1e-10; one JSON line of its own."""
+    import torch
+    from paper_2502_04189_b200.binding import Fizzy
+    torch.cuda.set_device(0)
+    cfg, f, dt, _ = W.make(args.workload, grid=tuple(args.grid) if args.grid else None)
+    cells = cfg["nx"] * cfg["ny"] * cfg["nz"]
+    fz = Fizzy(cfg, device="cuda:0")
+    fz.fizzy_set_fields(**{k: torch.from_numpy(f[k]).cuda() for k in ["u", "v", "w", "p", "phi"] + (["T"] if cfg["heat"] else [])})
+    rhs = torch.randn(cfg["nz"], cfg["ny"], cfg["nx"], dtype=torch.float64, device="cuda:0")
+    p = torch.empty_like(rhs)
+    it, rr = fz.fizzy_poisson_solve_varcoef(rhs, p, rtol=1e-10, max_iter=200)      # warm-up (allocates the scratch)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    n0 = fz.fizzy_launch_count()
+    e0.record(fz.stream)
+    it, rr = fz.fizzy_poisson_solve_varcoef(rhs, p, rtol=1e-10, max_iter=200)
+    e1.record(fz.stream)
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1)
+    e0.record(fz.stream)
+    fz.fizzy_poisson_solve(rhs, p)
+    e1.record(fz.stream)
+    torch.cuda.synchronize()
+    print(json.dumps({"metric": "variable-coefficient Poisson solve (multigrid-preconditioned CG, rtol 1e-10)", "workload": cfg["name"],
+                      "grid": [cfg["nx"], cfg["ny"], cfg["nz"]], "rho_ratio": max(cfg["rho1"], cfg["rho2"]) / min(cfg["rho1"], cfg["rho2"]),
+                      "iterations": it, "relres": rr, "ms": ms, "ms_per_iteration": ms / max(it, 1),
+                      "Mcell_per_s": cells / (ms * 1e-3) / 1e6, "gpu_launches": fz.fizzy_launch_count() - n0,
+                      "constant_coefficient_fft_solve_ms": e0.elapsed_time(e1)}), flush=True)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -269,7 +300,11 @@ def main():
     ap.add_argument("--no-cufft", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--varcoef", action="store_true", help="time fizzy_poisson_solve_varcoef (SURVEY 8(f)-4) instead of the RK3 step")
     args = ap.parse_args()
+    if args.varcoef:
+        varcoef_bench(args)
+        return
     args.warmup = max(args.warmup, 3) if args.impl == "fizzy" else args.warmup
 
     rank = int(os.environ.get("RANK", "0"))

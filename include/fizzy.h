@@ -147,6 +147,24 @@ fizzy_status fizzy_check_finite(fizzy_ctx *ctx, long long *count);
  * mean is removed.  rhs and p are N doubles, host or device; they may alias. */
 fizzy_status fizzy_poisson_solve(fizzy_ctx *ctx, const double *rhs, double *p);
 
+/* the conventional VARIABLE-COEFFICIENT pressure problem that PAPER.md:36 names as Fizzy's alternative to
+ * the splitting ("solving the conventional variable-coefficients problem using a geometric multigrid method"):
+ *     D( (1/rho_f) d_a p ) = rhs,   rho_f = 1/2 (rho + rho(+1_a)),  rho = rho[1] + (rho[0]-rho[1]) clip(phi,0,1)  (N2, N11),
+ * with the context's grid and z boundary condition (periodic x, y; periodic or no-flux walls in z; stretched z allowed).
+ * Solved by conjugate gradients preconditioned with one geometric multigrid V-cycle (red-black Gauss-Seidel, levels
+ * halving nx, ny, nz while all stay even and >= 4), to  ||rhs' - A p|| <= rtol ||rhs'||  in the dzf-weighted 2-norm, where
+ * rhs' = rhs minus its dzf-weighted mean (the operator is singular); p is returned with zero dzf-weighted mean (N17).
+ * rhs, p: N doubles, host or device.  phi: N doubles, host or device, or NULL = the context's current phase field.
+ * dev_work: caller-owned DEVICE scratch of fizzy_varcoef_workspace_bytes(ctx) bytes, 256-byte aligned (about 10 N
+ * doubles); nothing is kept in it between calls.  *iters (may be NULL) = CG iterations used, *relres (may be NULL) = the
+ * relative residual reached.  Synchronises the stream (the CG scalars are read on the host).
+ * FIZZY_EINVAL: NULL rhs / p / dev_work, rtol <= 0, max_iter < 1, misaligned dev_work.  FIZZY_ENOMEM: work_bytes too small.
+ * FIZZY_ESTATE: phi == NULL before fizzy_set_fields.  Not converged within max_iter is NOT an error: check *relres. */
+size_t fizzy_varcoef_workspace_bytes(const fizzy_ctx *ctx);
+fizzy_status fizzy_poisson_solve_varcoef(fizzy_ctx *ctx, const double *rhs, const double *phi, double *p,
+                                         void *dev_work, size_t work_bytes, double rtol, int max_iter,
+                                         int *iters, double *relres);
+
 /* Copy the prognostic fields out (same layout and meaning as fizzy_set_fields; host or device pointers); any
  * pointer may be NULL.  Enqueued on the stream like every other call: synchronise before reading host memory. */
 fizzy_status fizzy_get_fields(fizzy_ctx *ctx, double *u, double *v, double *w, double *p,

@@ -68,6 +68,11 @@ def load_library(path: str = LIB_PATH) -> C.CDLL:
     lib.fizzy_rk3_substep.argtypes = [vp, C.c_int, C.c_double]
     lib.fizzy_poisson_solve.restype = C.c_int
     lib.fizzy_poisson_solve.argtypes = [vp, dp, dp]
+    lib.fizzy_varcoef_workspace_bytes.restype = C.c_size_t
+    lib.fizzy_varcoef_workspace_bytes.argtypes = [vp]
+    lib.fizzy_poisson_solve_varcoef.restype = C.c_int
+    lib.fizzy_poisson_solve_varcoef.argtypes = [vp, dp, dp, dp, vp, C.c_size_t, C.c_double, C.c_int,
+                                                C.POINTER(C.c_int), C.POINTER(C.c_double)]
     lib.fizzy_diagnostics.restype = C.c_int
     lib.fizzy_diagnostics.argtypes = [vp, C.POINTER(C.c_double)]
     lib.fizzy_rk3_step.restype = C.c_int
@@ -200,6 +205,18 @@ class Fizzy:
     def fizzy_poisson_solve(self, rhs, p):
         with self._on_device():
             self._check(_lib.fizzy_poisson_solve(self._h, _addr(rhs), _addr(p)))
+
+    def fizzy_poisson_solve_varcoef(self, rhs, p, phi=None, rtol=1e-10, max_iter=100):
+        """Returns (iterations, relative residual).  The scratch tensor is torch-owned and kept for later calls."""
+        with self._on_device():
+            nbytes = _lib.fizzy_varcoef_workspace_bytes(self._h)
+            if getattr(self, "_vc_work", None) is None or self._vc_work.numel() < nbytes:
+                self._vc_work = self._torch.empty(nbytes, dtype=self._torch.uint8, device=self.device)
+            it, rr = C.c_int(), C.c_double()
+            self._check(_lib.fizzy_poisson_solve_varcoef(self._h, _addr(rhs), _addr(phi), _addr(p),
+                                                         self._vc_work.data_ptr(), nbytes, float(rtol), int(max_iter),
+                                                         C.byref(it), C.byref(rr)))
+        return it.value, rr.value
 
     def fizzy_diagnostics(self) -> np.ndarray:
         out = (C.c_double * 8)()

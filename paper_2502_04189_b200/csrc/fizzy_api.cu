@@ -16,6 +16,7 @@
 #include "fz_momentum.cuh"
 #include "fz_stencil.cuh"
 #include "fz_spectral.cuh"
+#include "fz_mg.cuh"
 
 namespace {
 
@@ -70,6 +71,7 @@ struct fizzy_ctx {
     double2 *twx, *twy;
     double *scal;  // [0] running max|u|, [1] Gamma, [2], [6] gauge mean (two parts), [3..4] dt maxima, [5] non-finite count, [8..15] diagnostics
     double dzmin;  // smallest cell height (N16)
+    std::vector<double> hdzf;   // host copy of dzf[0..nz-1] (level tables of fizzy_poisson_solve_varcoef)
     // one RK3 step as a CUDA graph (fizzy_graph_enable): one executable graph per parity of the step counter,
     // because phi/phi_new (and T/T_new) swap three times per step and are back in place after two steps
     bool graph_on = false;
@@ -300,6 +302,7 @@ extern "C" fizzy_status fizzy_create(const fizzy_grid *grid, const fizzy_bc *bc,
     for (int q = 0; q < nzt - 1; ++q) dzc[q] = 0.5 * (dzf[q] + dzf[q + 1]);
     dzc[nzt - 1] = dzc[nzt - 2];
     for (int q = 0; q < nzt; ++q) { idzf[q] = 1.0 / dzf[q]; idzc[q] = 1.0 / dzc[q]; }
+    c->hdzf.assign(dzf.begin() + FZ_H, dzf.begin() + FZ_H + nz);
     c->dzmin = dzf[FZ_H];
     for (int k = 0; k < nz; ++k) c->dzmin = std::fmin(c->dzmin, dzf[k + FZ_H]);
     for (int q = 1; q < nzt; ++q) igz[q] = 1.0 / (dzc[q] + dzc[q - 1]);
@@ -824,5 +827,202 @@ extern "C" fizzy_status fizzy_rk3_step(fizzy_ctx *c, double dt)
     std::swap(c->phi, c->phin);
     if (c->heat) std::swap(c->T, c->Tn);
     c->launches += c->glaunches[par];
+    return FIZZY_OK;
+}
+
+// =====================================================================================
+// variable-coefficient pressure Poisson problem, multigrid-preconditioned CG (fz_mg.cuh)
+namespace {
+
+struct MgPlan {
+    int nlev;
+    int nx[FZ_MG_MAXLEV], ny[FZ_MG_MAXLEV], nz[FZ_MG_MAXLEV];
+    size_t doubles;   // workspace, in doubles
+};
+
+// levels halve nx, ny, nz together while all three stay even and the coarse grid keeps >= 4 cells per direction
+MgPlan mg_plan(const fizzy_ctx *c)
+{
+    MgPlan m;
+    m.nlev = 1;
+    m.nx[0] = c->P.nx; m.ny[0] = c->P.ny; m.nz[0] = c->P.nz;
+    while (m.nlev < FZ_MG_MAXLEV) {
+        const int q = m.nlev - 1;
+        if ((m.nx[q] | m.ny[q] | m.nz[q]) & 1) break;
+        if (m.nx[q] < 8 || m.ny[q] < 8 || m.nz[q] < 8) break;
+        m.nx[m.nlev] = m.nx[q] / 2; m.ny[m.nlev] = m.ny[q] / 2; m.nz[m.nlev] = m.nz[q] / 2;
+        ++m.nlev;
+    }
+    size_t d = 9 * (size_t)c->N;   // sol, res, d, q | level 0: x, r, bx, by, bz (its b is res)
+    for (int q = 1; q < m.nlev; ++q) d += 6 * (size_t)m.nx[q] * m.ny[q] * m.nz[q];
+    for (int q = 0; q < m.nlev; ++q) d += 3 * (size_t)m.nz[q] + 32;
+    d += FZ_MG_RBLOCKS + 64;
+    m.doubles = d + 64 * (size_t)(6 * m.nlev + 16);   // 256-byte alignment slack of every piece
+    return m;
+}
+
+void mg_grid(const FzMgLevel &L, dim3 &grid, dim3 &block)
+{
+    block = dim3(32, 8, 1);
+    grid = dim3((L.nx + 31) / 32, (L.ny + 7) / 8, L.nz);
+}
+
+}  // namespace
+
+extern "C" size_t fizzy_varcoef_workspace_bytes(const fizzy_ctx *c)
+{
+    return c ? mg_plan(c).doubles * sizeof(double) : 0;
+}
+
+extern "C" fizzy_status fizzy_poisson_solve_varcoef(fizzy_ctx *c, const double *rhs, const double *phi, double *p,
+                                                    void *dev_work, size_t work_bytes, double rtol, int max_iter,
+                                                    int *iters, double *relres)
+{
+    if (!c) return FIZZY_EINVAL;
+    FZ_DEVICE();
+    if (!rhs || !p || !dev_work || !(rtol > 0.0) || max_iter < 1) return fail(c, FIZZY_EINVAL, "rhs, p, dev_work must be non-NULL, rtol > 0, max_iter >= 1");
+    if (reinterpret_cast<uintptr_t>(dev_work) & 255) return fail(c, FIZZY_EINVAL, "dev_work must be 256-byte aligned");
+    const MgPlan plan = mg_plan(c);
+    if (work_bytes < plan.doubles * sizeof(double)) return fail(c, FIZZY_ENOMEM, "dev_work is smaller than fizzy_varcoef_workspace_bytes");
+    if (!phi && !c->fields_set) return fail(c, FIZZY_ESTATE, "phi == NULL needs fizzy_set_fields first");
+    const FzP &P = c->P;
+    const int n = (int)c->N;
+    cudaStream_t st = c->stream;
+    Carver cv(dev_work);
+    double *sol = cv.dbl(n), *res = cv.dbl(n), *dir = cv.dbl(n), *q = cv.dbl(n);
+    FzMgLevel L[FZ_MG_MAXLEV];
+    std::vector<double> tab;
+    for (int l = 0; l < plan.nlev; ++l) {
+        const size_t nl = (size_t)plan.nx[l] * plan.ny[l] * plan.nz[l];
+        L[l].nx = plan.nx[l]; L[l].ny = plan.ny[l]; L[l].nz = plan.nz[l]; L[l].z_wall = P.z_wall;
+        const double dx = P.dx * (1 << l), dy = P.dy * (1 << l);
+        L[l].cx = 1.0 / (dx * dx); L[l].cy = 1.0 / (dy * dy);
+        L[l].x = cv.dbl(nl);
+        L[l].b = l == 0 ? res : cv.dbl(nl);
+        L[l].r = cv.dbl(nl);
+        L[l].bx = cv.dbl(nl); L[l].by = cv.dbl(nl); L[l].bz = cv.dbl(nl);
+    }
+    // 1-D z tables of every level: dzf (sum of the two children), centre spacings from face midpoints (N10)
+    std::vector<double> dz = c->hdzf;
+    for (int l = 0; l < plan.nlev; ++l) {
+        const int nzl = plan.nz[l];
+        if (l > 0) { std::vector<double> cz(nzl); for (int k = 0; k < nzl; ++k) cz[k] = dz[2 * k] + dz[2 * k + 1]; dz.swap(cz); }
+        std::vector<double> t(3 * (size_t)nzl);
+        for (int k = 0; k < nzl; ++k) {
+            const int kp = k + 1 == nzl ? 0 : k + 1, km = k == 0 ? nzl - 1 : k - 1;
+            const double dzc_p = 0.5 * (dz[k] + dz[kp]), dzc_m = 0.5 * (dz[km] + dz[k]);
+            t[k] = dz[k];
+            t[nzl + k] = (P.z_wall && k == nzl - 1) ? 0.0 : 1.0 / (dzc_p * dz[k]);
+            t[2 * nzl + k] = (P.z_wall && k == 0) ? 0.0 : 1.0 / (dzc_m * dz[k]);
+        }
+        double *dt = cv.dbl(3 * (size_t)nzl);
+        FZ_CUDA(cudaMemcpyAsync(dt, t.data(), t.size() * sizeof(double), cudaMemcpyHostToDevice, st));
+        FZ_CUDA(cudaStreamSynchronize(st));   // t goes out of scope
+        L[l].wz = dt; L[l].czh = dt + nzl; L[l].czl = dt + 2 * nzl;
+    }
+    double *partial = cv.dbl(FZ_MG_RBLOCKS), *scalar = cv.dbl(8);
+    dim3 grid, block;
+
+    // face coefficients of every level
+    const double *dphi = c->phi;
+    if (phi) {   // a caller-supplied phase field: stage it in `q` (free until the CG loop)
+        FZ_CUDA(cudaMemcpyAsync(q, phi, (size_t)n * sizeof(double), cudaMemcpyDefault, st));
+        dphi = q;
+    }
+    mg_grid(L[0], grid, block);
+    k_mg_beta<<<grid, block, 0, st>>>(L[0], dphi, P.rho2, P.drho);
+    ++c->launches;
+    for (int l = 1; l < plan.nlev; ++l) {
+        mg_grid(L[l], grid, block);
+        k_mg_coarsen_beta<<<grid, block, 0, st>>>(L[l], L[l - 1]);
+        ++c->launches;
+    }
+    FZ_CUDA(cudaPeekAtLastError());
+
+    const int plane = P.nx * P.ny;
+    auto dotw = [&](const double *a, const double *b, double *out) -> cudaError_t {
+        k_mg_dot<<<FZ_MG_RBLOCKS, 256, 0, st>>>(a, b, L[0].wz, plane, n, partial);
+        k_mg_dot_final<<<1, 256, 0, st>>>(partial, FZ_MG_RBLOCKS, scalar);
+        c->launches += 2;
+        cudaError_t e = cudaMemcpyAsync(out, scalar, sizeof(double), cudaMemcpyDeviceToHost, st);
+        return e == cudaSuccess ? cudaStreamSynchronize(st) : e;
+    };
+    auto smooth = [&](const FzMgLevel &lev, int sweeps, bool forward) {
+        dim3 g2, b2;
+        mg_grid(lev, g2, b2);
+        for (int s = 0; s < sweeps; ++s) {
+            k_mg_gs<<<g2, b2, 0, st>>>(lev, forward ? 0 : 1);
+            k_mg_gs<<<g2, b2, 0, st>>>(lev, forward ? 1 : 0);
+            c->launches += 2;
+        }
+    };
+    // z = V-cycle approximation of A^-1 res, into L[0].x
+    auto vcycle = [&]() {
+        dim3 g2, b2;
+        k_mg_fill<<<FZ_MG_RBLOCKS, 256, 0, st>>>(L[0].x, 0.0, n);
+        ++c->launches;
+        for (int l = 0; l < plan.nlev - 1; ++l) {
+            smooth(L[l], FZ_MG_NU, true);
+            mg_grid(L[l], g2, b2);
+            k_mg_residual<<<g2, b2, 0, st>>>(L[l]);
+            mg_grid(L[l + 1], g2, b2);
+            k_mg_restrict<<<g2, b2, 0, st>>>(L[l + 1], L[l]);
+            c->launches += 2;
+        }
+        smooth(L[plan.nlev - 1], FZ_MG_COARSE, true);
+        smooth(L[plan.nlev - 1], FZ_MG_COARSE, false);
+        for (int l = plan.nlev - 2; l >= 0; --l) {
+            mg_grid(L[l], g2, b2);
+            k_mg_prolong<<<g2, b2, 0, st>>>(L[l], L[l + 1]);
+            ++c->launches;
+            smooth(L[l], FZ_MG_NU, false);
+        }
+    };
+
+    // res = rhs - (dzf-weighted mean of rhs); sol = 0
+    FZ_CUDA(cudaMemcpyAsync(res, rhs, (size_t)n * sizeof(double), cudaMemcpyDefault, st));
+    double s1 = 0.0, vol = 0.0, bb = 0.0;
+    k_mg_fill<<<FZ_MG_RBLOCKS, 256, 0, st>>>(sol, 1.0, n);
+    FZ_CUDA(dotw(sol, nullptr, &vol));
+    FZ_CUDA(dotw(res, nullptr, &s1));
+    k_mg_shift<<<FZ_MG_RBLOCKS, 256, 0, st>>>(res, res, -s1 / vol, n);
+    k_mg_fill<<<FZ_MG_RBLOCKS, 256, 0, st>>>(sol, 0.0, n);
+    c->launches += 3;
+    FZ_CUDA(dotw(res, res, &bb));
+    int it = 0;
+    double rr = bb;
+    if (bb > 0.0) {
+        double rz = 0.0, rz_new = 0.0, dq = 0.0;
+        vcycle();
+        FZ_CUDA(cudaMemcpyAsync(dir, L[0].x, (size_t)n * sizeof(double), cudaMemcpyDeviceToDevice, st));
+        FZ_CUDA(dotw(res, L[0].x, &rz));
+        mg_grid(L[0], grid, block);
+        for (it = 1; it <= max_iter; ++it) {
+            k_mg_apply<<<grid, block, 0, st>>>(L[0], dir, q);
+            ++c->launches;
+            FZ_CUDA(dotw(dir, q, &dq));
+            if (!(dq != 0.0) || !std::isfinite(dq)) return fail(c, FIZZY_ECUDA, "fizzy_poisson_solve_varcoef: breakdown (d, A d) = 0 or not finite");
+            const double alpha = rz / dq;
+            k_mg_axpby<<<FZ_MG_RBLOCKS, 256, 0, st>>>(sol, dir, alpha, 1.0, n);
+            k_mg_axpby<<<FZ_MG_RBLOCKS, 256, 0, st>>>(res, q, -alpha, 1.0, n);
+            c->launches += 2;
+            FZ_CUDA(dotw(res, res, &rr));
+            if (rr <= rtol * rtol * bb) break;
+            vcycle();
+            FZ_CUDA(dotw(res, L[0].x, &rz_new));
+            k_mg_axpby<<<FZ_MG_RBLOCKS, 256, 0, st>>>(dir, L[0].x, 1.0, rz_new / rz, n);
+            ++c->launches;
+            rz = rz_new;
+        }
+        if (it > max_iter) it = max_iter;
+    }
+    // gauge N17: remove the dzf-weighted mean, copy out
+    FZ_CUDA(dotw(sol, nullptr, &s1));
+    k_mg_shift<<<FZ_MG_RBLOCKS, 256, 0, st>>>(sol, sol, -s1 / vol, n);
+    ++c->launches;
+    FZ_CUDA(cudaPeekAtLastError());
+    FZ_CUDA(cudaMemcpyAsync(p, sol, (size_t)n * sizeof(double), cudaMemcpyDefault, st));
+    if (iters) *iters = it;
+    if (relres) *relres = bb > 0.0 ? std::sqrt(rr / bb) : 0.0;
     return FIZZY_OK;
 }

@@ -19,7 +19,8 @@ _STATUS = {0: "FIZZY_OK", 1: "FIZZY_EINVAL", 2: "FIZZY_ENOMEM", 3: "FIZZY_ECUDA"
 EXPORTS = ["fizzy_workspace_bytes", "fizzy_create", "fizzy_destroy", "fizzy_set_fields",
            "fizzy_rk3_substep", "fizzy_poisson_solve", "fizzy_get_fields", "fizzy_gamma", "fizzy_diagnostics",
            "fizzy_launch_count", "fizzy_last_error", "fizzy_timing_enable", "fizzy_timing_get",
-           "fizzy_rk3_step", "fizzy_graph_enable", "fizzy_stable_dt", "fizzy_check_finite"]
+           "fizzy_rk3_step", "fizzy_graph_enable", "fizzy_stable_dt", "fizzy_check_finite",
+           "fizzy_varcoef_workspace_bytes", "fizzy_poisson_solve_varcoef"]
 
 
 class FizzyGrid(C.Structure):

@@ -6,7 +6,8 @@
 // stretched z allowed.  Row k of the operator carries 1/dzf[k], so A is self-adjoint and negative semi-definite in the
 // dzf-weighted inner product <u,v> = sum dzf[k] u v; constants span its null space (gauge N17: <1,p> = 0, and the
 // dzf-weighted mean of rhs is removed first).  Every ingredient keeps that symmetry, which CG needs:
-//   * smoother: red-black Gauss-Seidel, colours in the order R,B before and B,R after the coarse-grid correction;
+//   * smoother: red-black Gauss-Seidel, colours in the order R,B before and B,R after the coarse-grid correction
+//     (zebra z-line Gauss-Seidel instead on wall-bounded grids with flat cells, see k_mg_zline);
 //   * restriction: volume-weighted mean of the 8 children; prolongation: piecewise constant (its weighted adjoint);
 //   * coarse operators: the same discretisation on the coarse grid, face coefficient = mean of the 4 fine faces that
 //     tile the coarse face; levels halve nx, ny, nz together while all three stay even and >= 4;
@@ -96,6 +97,42 @@ __global__ void k_mg_gs(FzMgLevel L, int colour)
     FZ_MG_COEF
     const double s = axp * L.x[ip] + axm * L.x[im] + ayp * L.x[jp] + aym * L.x[jm] + azp * L.x[kp] + azm * L.x[km];
     L.x[c] = (s - L.b[c]) / (axp + axm + ayp + aym + azp + azm);
+}
+
+// z-line ("zebra") Gauss-Seidel for wall-bounded z: one thread per column (i, j) with (i + j) & 1 == colour solves the
+// tridiagonal system of its nz unknowns exactly (Thomas; the x and y neighbours belong to the other colour and are
+// frozen).  On the stretched wall grids the z coupling is 6-30 times the x, y coupling near the walls and point
+// relaxation stalls (71 CG iterations at 512 x 256 x 256 of config 5); relaxing whole z lines restores the textbook
+// rate.  Scratch: L.r holds the eliminated super-diagonal, L.x the modified right-hand side, then the solution.
+__global__ void k_mg_zline(FzMgLevel L, int colour)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int j = blockIdx.y * blockDim.y + threadIdx.y;
+    if (i >= L.nx || j >= L.ny || (((i + j) & 1) != colour)) return;
+    const int sxy = L.nx * L.ny, c0 = i + L.nx * j;
+    const int im = c0 - i + (i == 0 ? L.nx - 1 : i - 1), ip = c0 - i + (i + 1 == L.nx ? 0 : i + 1);
+    const int jm = c0 + ((j == 0 ? L.ny - 1 : j - 1) - j) * L.nx, jp = c0 + ((j + 1 == L.ny ? 0 : j + 1) - j) * L.nx;
+    double cp = 0.0, dp = 0.0, bzm = 0.0;   // c'_{k-1}, d'_{k-1}, bz of the face below (no flux through the bottom wall)
+    for (int k = 0; k < L.nz; ++k) {
+        const int o = k * sxy, c = c0 + o;
+        const double axp = L.cx * L.bx[c], axm = L.cx * L.bx[im + o], ayp = L.cy * L.by[c], aym = L.cy * L.by[jm + o];
+        const double bzc = L.bz[c];
+        const double azp = L.czh[k] * bzc, azm = L.czl[k] * bzm;
+        const double diag = -(axp + axm + ayp + aym + azp + azm);
+        const double rhs = L.b[c] - (axp * L.x[ip + o] + axm * L.x[im + o] + ayp * L.x[jp + o] + aym * L.x[jm + o]);
+        const double inv = 1.0 / (diag - azm * cp);
+        cp = azp * inv;
+        dp = (rhs - azm * dp) * inv;
+        L.r[c] = cp;
+        L.x[c] = dp;
+        bzm = bzc;
+    }
+    double xn = 0.0;
+    for (int k = L.nz - 1; k >= 0; --k) {
+        const int c = c0 + k * sxy;
+        xn = L.x[c] - L.r[c] * xn;
+        L.x[c] = xn;
+    }
 }
 
 // b_coarse = volume-weighted mean of the residual of the 8 children; x_coarse = 0   (L = coarse, F = fine)

@@ -24,7 +24,15 @@ struct FzP {
     double rho0, drho;         // min(rho1, rho2), rho1 - rho2
 };
 
-__device__ __forceinline__ double fz_clip01(double f) { return fmin(fmax(f, 0.0), 1.0); }
+// clip(f, 0, 1) on the bit pattern: f < 0 (sign bit) -> 0, f >= 1 (high word >= that of 1.0) -> 1, else f.  Equal to
+// fmin(fmax(f, 0), 1) for every non-NaN f, in two integer compares and three selects; fmin/fmax cost a DSETP, two
+// selects, a NaN fix-up and several moves each (14 instructions per clip in k_iface_march, two of them on the fp64 pipe).
+__device__ __forceinline__ double fz_clip01(double f)
+{
+    const int hi = __double2hiint(f), lo = __double2loint(f);
+    const bool neg = hi < 0, big = hi >= 0x3ff00000;
+    return __hiloint2double(neg ? 0 : (big ? 0x3ff00000 : hi), (neg || big) ? 0 : lo);
+}
 // 2 clip(f,0,1) - 1 = |f| - |f - 1| without a comparison (two DADD with operand modifiers instead of DSETP + selects
 // + moves per fmin/fmax): exact outside [0,1], within one rounding of 1 (1.1e-16 ABSOLUTE) inside.  For the linear
 // property maps q2 + (q1-q2) clip(phi) = (q2+q1)/2 + (q1-q2)/2 * fz_sclip(phi), where an absolute error of that size

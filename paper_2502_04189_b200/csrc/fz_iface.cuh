@@ -108,7 +108,10 @@ k_iface_march(FzP P, const double *__restrict__ psi, const double *__restrict__ 
         const double gx = (q[o0 + 1] - q[o0 - 1]) * hx;
         const double gy = (q[o0 + IPW] - q[o0 - IPW]) * hy;
         const double gz = (q[op] - q[om]) * igz;
-        const double inv = 0.5 * fz_rsqrt(fmax(gx * gx + gy * gy + gz * gz, 1e-60));
+        // max(|G|^2, 1e-60) for a non-negative, non-NaN |G|^2: ordered like its bit pattern (fmax costs ten instructions)
+        double g2 = gx * gx + gy * gy + gz * gz;
+        if (__double_as_longlong(g2) < __double_as_longlong(1e-60)) g2 = 1e-60;
+        const double inv = 0.5 * fz_rsqrt(g2);
         nx_ = gx * inv; ny_ = gy * inv; nz_ = gz * inv;
     };
 
@@ -150,10 +153,11 @@ k_iface_march(FzP P, const double *__restrict__ psi, const double *__restrict__ 
         const int k = kk - 1;
         if (k < k0 - 1) return;
         const double f0 = PHIc[om], r0 = RRc[rm];
-        // z face k+1/2: zero on a wall face; the face k-1/2 is carried in registers
-        const double zf = (P.z_wall && (k == -1 || k == P.nz - 1)) ? 0.0 : 1.0;
-        const double nfzp = zf * (nz0 + nzp);
-        const double Rzp = zf * (P.eps * (PHIc[o0] - f0) * idzc_k - fz_sharp2(r0, RRc[r0s]) * nfzp);
+        // z face k+1/2; the face k-1/2 is carried in registers.  On a wall face both terms vanish by themselves, exactly:
+        // the ghost planes hold the mirrored psi and phi (and igz is mirrored), so nhat_z of the ghost cell is bit for bit
+        // minus that of the wall cell (nf_z = 0, N3/walls) and phi(ghost) - phi(wall cell) = 0 (R_z = 0)
+        const double nfzp = nz0 + nzp;
+        const double Rzp = P.eps * (PHIc[o0] - f0) * idzc_k - fz_sharp2(r0, RRc[r0s]) * nfzp;
         if (k < k0) { nfz_prev = nfzp; Rz_prev = Rzp; return; }
         // half normals of plane k were written one step ago: visible after this step's barrier
         const double ax = NHXc[nm], ay = NHYc[nm];

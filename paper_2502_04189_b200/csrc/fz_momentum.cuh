@@ -236,7 +236,7 @@ k_momentum_march(FzP P, FzMomArgs A, int KC)
     const int i = i0 + tx, j = j0 + ty;
     const int k0 = blockIdx.z * KC, k1 = min(k0 + KC, P.nz);
     const int cidx = (ty + 1) * MPW + (tx + 2);
-    const long long goff_c = i + (long long)P.nx * j;
+    const unsigned ugc = (unsigned)(i + P.nx * j);   // 32-bit cell offsets: N < 2^31 (fizzy_create)
     // staging map: thread t < MCHUNKS copies 16-byte chunk t of the staged rectangle of every field
     const bool loader = t < MCHUNKS;
     const int lrow = t / (MPW / 2), lcp = t - lrow * (MPW / 2);
@@ -282,8 +282,8 @@ k_momentum_march(FzP P, FzMomArgs A, int KC)
     const bool use_h = A.zs != 0.0;
     double hu_nx = 0.0, hv_nx = 0.0, hw_nx = 0.0;
     if (use_h) {
-        hu_nx = A.hu[(long long)k0 * P.sxy + goff_c]; hv_nx = A.hv[(long long)k0 * P.sxy + goff_c];
-        hw_nx = A.hw[(long long)k0 * P.sxy + goff_c];
+        hu_nx = A.hu[(unsigned)k0 * sxy + ugc]; hv_nx = A.hv[(unsigned)k0 * sxy + ugc];
+        hw_nx = A.hw[(unsigned)k0 * sxy + ugc];
     }
     double izc_0 = P.idzc[k0 - 1], izc_n = P.idzc[k0], izf_p = P.idzf[k0], izf_n = P.idzf[k0 + 1];
     for (int k = k0; k < k1; ++k) {
@@ -293,13 +293,26 @@ k_momentum_march(FzP P, FzMomArgs A, int KC)
         fz_cp_async_commit();
         sl = (sl + 1 == MRING) ? 0 : sl + 1;
         om = o0; o0 = op; op = sl * MPS + cidx;   // planes k-1, k, k+1
-        const long long c = (long long)k * P.sxy + goff_c;
+        const unsigned c = (unsigned)k * sxy + ugc;
         // RK histories: loaded one plane ahead (registers), so their latency hides behind a whole plane
         const double hu_old = hu_nx, hv_old = hv_nx, hw_old = hw_nx;
-        if (use_h && k + 1 < k1) { hu_nx = A.hu[c + P.sxy]; hv_nx = A.hv[c + P.sxy]; hw_nx = A.hw[c + P.sxy]; }
-        // ghost rules at the walls: planes k-1 / k+1 hold the mirrored interior plane
-        const bool gm = P.z_wall && k == 0, gp = P.z_wall && k == P.nz - 1;
-        const double sgm = gm ? -1.0 : 1.0, sgp = gp ? -1.0 : 1.0, wm = gm ? 0.0 : 1.0;
+        if (use_h && k + 1 < k1) { hu_nx = A.hu[c + sxy]; hv_nx = A.hv[c + sxy]; hw_nx = A.hw[c + sxy]; }
+        // ghost rules at the walls: the ring slot of plane -1 / nz arrives holding the mirrored interior plane; the two
+        // plane steps that read it turn it into the ghost plane first (no-slip: -u, -v; impermeable: w = 0, R_z = 0; phi,
+        // kappa, p_hat, T are even and stay), so that the other nz-2 steps -- and every step of a periodic grid -- carry no
+        // sign factors (round 2: nine DMUL and a dozen select / predicate instructions per cell, in every configuration)
+        if (P.z_wall && (k == 0 || k == P.nz - 1)) {
+            const int gb = (k == 0 ? om : op) - cidx;
+            for (int e = t; e < MPS; e += MTX * MTY) {
+                smm[F::U * (MRING * MPS) + gb + e] = -smm[F::U * (MRING * MPS) + gb + e];
+                smm[F::V * (MRING * MPS) + gb + e] = -smm[F::V * (MRING * MPS) + gb + e];
+                if (k == 0) {
+                    smm[F::W * (MRING * MPS) + gb + e] = 0.0;
+                    if (VARRHO) smm[F::RZ * (MRING * MPS) + gb + e] = 0.0;
+                }
+            }
+            __syncthreads();
+        }
         // S(f, di, dj, plane offset) -- shared-memory neighbour read
 #define S_(f, di, dj, o) smm[(f) * (MRING * MPS) + (o) + (dj) * MPW + (di)]   // o includes cidx
         // z metrics come from global tables: carried / loaded one plane ahead so that no plane waits for them
@@ -309,13 +322,13 @@ k_momentum_march(FzP P, FzMomArgs A, int KC)
         const double izfp = izf_p;   // 1/dzf[k+1]
         const double u000 = S_(F::U, 0, 0, o0), up00 = S_(F::U, 1, 0, o0), um00 = S_(F::U, -1, 0, o0);
         const double u0p0 = S_(F::U, 0, 1, o0), u0m0 = S_(F::U, 0, -1, o0), ump0 = S_(F::U, -1, 1, o0);
-        const double u00p = sgp * S_(F::U, 0, 0, op), u00m = sgm * S_(F::U, 0, 0, om), um0p = sgp * S_(F::U, -1, 0, op);
+        const double u00p = S_(F::U, 0, 0, op), u00m = S_(F::U, 0, 0, om), um0p = S_(F::U, -1, 0, op);
         const double v000 = S_(F::V, 0, 0, o0), vp00 = S_(F::V, 1, 0, o0), vm00 = S_(F::V, -1, 0, o0);
         const double v0p0 = S_(F::V, 0, 1, o0), v0m0 = S_(F::V, 0, -1, o0), vpm0 = S_(F::V, 1, -1, o0);
-        const double v00p = sgp * S_(F::V, 0, 0, op), v00m = sgm * S_(F::V, 0, 0, om), v0mp = sgp * S_(F::V, 0, -1, op);
+        const double v00p = S_(F::V, 0, 0, op), v00m = S_(F::V, 0, 0, om), v0mp = S_(F::V, 0, -1, op);
         const double w000 = S_(F::W, 0, 0, o0), wp00 = S_(F::W, 1, 0, o0), wm00 = S_(F::W, -1, 0, o0);
         const double w0p0 = S_(F::W, 0, 1, o0), w0m0 = S_(F::W, 0, -1, o0);
-        const double w00m = wm * S_(F::W, 0, 0, om), wp0m = wm * S_(F::W, 1, 0, om), w0pm = wm * S_(F::W, 0, 1, om);
+        const double w00m = S_(F::W, 0, 0, om), wp0m = S_(F::W, 1, 0, om), w0pm = S_(F::W, 0, 1, om);
         const double f000 = S_(F::PHI, 0, 0, o0), fp00 = S_(F::PHI, 1, 0, o0), f0p0 = S_(F::PHI, 0, 1, o0),
                      f00p = S_(F::PHI, 0, 0, op);
         double m000, mp00, mm00, m0p0, m0m0, m00p, m00m, mpp0, mpm0, mmp0, mp0p, mp0m, mm0p, m0pp, m0pm, m0mp;
@@ -383,7 +396,7 @@ k_momentum_march(FzP P, FzMomArgs A, int KC)
             double M = 0.0;
             if (VARRHO) {
                 const double Rty = 0.25 * (S_(F::RY, 0, 0, o0) + S_(F::RY, 1, 0, o0) + S_(F::RY, 0, -1, o0) + S_(F::RY, 1, -1, o0));
-                const double Rtz = 0.25 * (S_(F::RZ, 0, 0, o0) + S_(F::RZ, 1, 0, o0) + wm * (S_(F::RZ, 0, 0, om) + S_(F::RZ, 1, 0, om)));
+                const double Rtz = 0.25 * (S_(F::RZ, 0, 0, o0) + S_(F::RZ, 1, 0, o0) + S_(F::RZ, 0, 0, om) + S_(F::RZ, 1, 0, om));
                 M = P.drho * Gam * (S_(F::RX, 0, 0, o0) * (up00 - um00) * (0.5 * dx) + Rty * (u0p0 - u0m0) * (0.5 * dy) +
                                     Rtz * (u00p - u00m) * P.igz[k]);
             }
@@ -411,7 +424,7 @@ k_momentum_march(FzP P, FzMomArgs A, int KC)
             double M = 0.0;
             if (VARRHO) {
                 const double Rtx = 0.25 * (S_(F::RX, 0, 0, o0) + S_(F::RX, 0, 1, o0) + S_(F::RX, -1, 0, o0) + S_(F::RX, -1, 1, o0));
-                const double Rtz = 0.25 * (S_(F::RZ, 0, 0, o0) + S_(F::RZ, 0, 1, o0) + wm * (S_(F::RZ, 0, 0, om) + S_(F::RZ, 0, 1, om)));
+                const double Rtz = 0.25 * (S_(F::RZ, 0, 0, o0) + S_(F::RZ, 0, 1, o0) + S_(F::RZ, 0, 0, om) + S_(F::RZ, 0, 1, om));
                 M = P.drho * Gam * (S_(F::RY, 0, 0, o0) * (v0p0 - v0m0) * (0.5 * dy) + Rtx * (vp00 - vm00) * (0.5 * dx) +
                                     Rtz * (v00p - v00m) * P.igz[k]);
             }

@@ -54,6 +54,31 @@ def test_varcoef_solve_matches_the_sparse_direct_oracle(fz, name):
     g.close()
 
 
+@pytest.mark.parametrize("index", [2, 4])
+def test_varcoef_full_size_residual_by_the_oracle_operator(fz, index):
+    """At sizes no sparse direct solve reaches (config 3 at its own 256^3, density ratio 1000, point relaxation; config
+    5's stretched channel at 512 x 256 x 256, z-line relaxation) the property that holds at any size: the returned p,
+    put through the ORACLE's operator (plain array differences), reproduces rhs minus its weighted mean to the tolerance
+    asked for, and has zero dzf-weighted mean."""
+    from oracle import varcoef as V
+    cfg, f, dt, _ = W.make(index, grid=None if index == 2 else (512, 256, 256), ndrops=None if index == 2 else 8)
+    shape = (cfg["nz"], cfg["ny"], cfg["nx"])
+    rhs = np.random.default_rng(8).standard_normal(shape)
+    g = fz.Fizzy(cfg)
+    p = np.empty(shape)
+    it, rr = g.fizzy_poisson_solve_varcoef(np.ascontiguousarray(rhs), p, phi=np.ascontiguousarray(f["phi"]), rtol=1e-10, max_iter=200)
+    g.stream.synchronize()
+    g.close()
+    assert rr <= 1e-10 and it < 60, (it, rr)
+    dzf, _ = V.z_metrics(cfg)
+    w = dzf[:, None, None]
+    wmean = lambda a: (a * w).sum() / (dzf.sum() * cfg["nx"] * cfg["ny"])
+    b = rhs - wmean(rhs)
+    res = V.apply(cfg, f["phi"], p) - b
+    assert np.sqrt((w * res * res).sum() / (w * b * b).sum()) <= 2e-10
+    assert abs(wmean(p)) <= 1e-12 * np.abs(p).max()
+
+
 def test_varcoef_constant_density_equals_the_fft_solver(fz):
     """rho1 = rho2: the multigrid solve and the direct FFT/tridiagonal solve of the same context agree."""
     cfg, f, dt, _ = W.make(1, grid=(64, 32, 16), ndrops=1)

@@ -69,6 +69,9 @@ def _load():
         lib.orc_substep.argtypes = [C.c_void_p, C.c_int, C.c_double]
         lib.orc_substep.restype = C.c_int
         lib.orc_poisson_solve.argtypes = [C.c_void_p, _dp, _dp]
+        lib.orc_set_solver.argtypes = [C.c_void_p, C.c_int]
+        lib.orc_varcoef_solve.argtypes = [C.c_void_p, _dp, _dp]
+        lib.orc_varcoef_solve.restype = C.c_int
         lib.orc_diagnostics.argtypes = [C.c_void_p, _dp]
         lib.orc_stable_dt.argtypes = [C.c_void_p, C.c_double]
         lib.orc_stable_dt.restype = C.c_double
@@ -156,6 +159,16 @@ class Oracle:
         rhs = _c(rhs)
         out = np.empty(self.shape)
         _load().orc_poisson_solve(self._h, _ptr(rhs), _ptr(out))
+        return out
+
+    def set_solver(self, solver: int):
+        """0: the constant-coefficient splitting; 1: the variable-coefficient problem."""
+        _load().orc_set_solver(self._h, int(solver))
+
+    def varcoef_solve(self, rhs) -> np.ndarray:
+        rhs = _c(rhs)
+        out = np.empty(self.shape)
+        self.varcoef_iterations = _load().orc_varcoef_solve(self._h, _ptr(rhs), _ptr(out))
         return out
 
     def diagnostics(self) -> np.ndarray:

@@ -38,6 +38,7 @@ struct orc_state {
     double *dzf_, *dzc_;   /* with ghost entries; use DZF(k), DZC(k) */
     double gamma;
     int fields_set;
+    int solver;            /* 0: constant-coefficient splitting (S4, S5 of BASELINE.json:5); 1: variable-coefficient problem */
     /* prognostic fields (padded) */
     double *u, *v, *w, *p, *pp, *phi, *T;
     /* RK history (padded, interior used) */
@@ -748,6 +749,125 @@ void orc_poisson_solve(orc_state *st, const double *rhs, double *p) { poisson_so
 
 /* ------------------------------------------------------------------ the substep
  * Low-storage RK3 (N1, Wray): f <- f + dt*(gamma_s RHS + zeta_s RHS_old), alpha = gamma+zeta */
+/* ------------------------------------------------------------------------------------------------
+ * SURVEY.md 8(f)-4, PAPER.md:36 ("the conventional variable-coefficients problem"): instead of the splitting,
+ *     D( (1/rho_f) d_a p ) = rhs,   rho_f = 1/2 (rho + rho(+1_a))  (N11),
+ * solved here by plain conjugate gradients (no preconditioner) in the dzf-weighted inner product, in which the
+ * operator is self-adjoint; the dzf-weighted mean of rhs is removed first (the operator is singular) and the
+ * solution returned with zero dzf-weighted mean (the gauge of N17).  An iteration, so the oracle follows it step by
+ * step; what it converges to is pinned against the sparse direct solve of oracle/varcoef.py. */
+static void varcoef_apply(orc_state *st, double *x, double *out)
+{
+    const int nx = st->nx, ny = st->ny, nz = st->nz, kzf = nzw(st);
+    const double dx = st->dx, dy = st->dy;
+    const double *rho = st->rho;
+    fill_ghosts(st, x, BC_EVEN, 0, 0);
+#pragma omp parallel for
+    for (int k = 0; k < nz; ++k)
+        for (int j = 0; j < ny; ++j)
+            for (int i = 0; i < nx; ++i) {
+                size_t c = IDX(i, j, k);
+                st->Fx[c] = (x[IDX(i + 1, j, k)] - x[c]) / dx / (0.5 * (rho[c] + rho[IDX(i + 1, j, k)]));
+                st->Fy[c] = (x[IDX(i, j + 1, k)] - x[c]) / dy / (0.5 * (rho[c] + rho[IDX(i, j + 1, k)]));
+                st->Fz[c] = (k < kzf) ? (x[IDX(i, j, k + 1)] - x[c]) / DZC(k) / (0.5 * (rho[c] + rho[IDX(i, j, k + 1)])) : 0.0;
+            }
+    fill_ghosts(st, st->Fx, BC_EVEN, 0, 0);
+    fill_ghosts(st, st->Fy, BC_EVEN, 0, 0);
+    fill_ghosts(st, st->Fz, BC_WFACE, 0, 0);
+#pragma omp parallel for
+    for (int k = 0; k < nz; ++k)
+        for (int j = 0; j < ny; ++j)
+            for (int i = 0; i < nx; ++i) {
+                size_t c = IDX(i, j, k);
+                out[c] = (st->Fx[c] - st->Fx[IDX(i - 1, j, k)]) / dx + (st->Fy[c] - st->Fy[IDX(i, j - 1, k)]) / dy +
+                         (st->Fz[c] - st->Fz[IDX(i, j, k - 1)]) / DZF(k);
+            }
+}
+
+static double wdot(const orc_state *st, const double *a, const double *b)
+{
+    double s = 0.0;
+    for (int k = 0; k < st->nz; ++k) {
+        double sk = 0.0;
+        for (int j = 0; j < st->ny; ++j)
+            for (int i = 0; i < st->nx; ++i) sk += a[IDX(i, j, k)] * (b ? b[IDX(i, j, k)] : 1.0);
+        s += DZF(k) * sk;
+    }
+    return s;
+}
+
+/* b (padded, interior used; overwritten by the final residual), x (padded): x = solution with zero weighted mean */
+static int varcoef_solve(orc_state *st, double *b, double *x)
+{
+    const int nx = st->nx, ny = st->ny, nz = st->nz;
+    double *d = palloc(st), *q = palloc(st);
+    double V = 0.0;
+    for (int k = 0; k < nz; ++k) V += DZF(k) * nx * ny;
+    /* remove the weighted mean of the right-hand side; x = 0; r = b; d = r */
+    double mb = 0.0;
+    for (int k = 0; k < nz; ++k)
+        for (int j = 0; j < ny; ++j)
+            for (int i = 0; i < nx; ++i) mb += DZF(k) * b[IDX(i, j, k)];
+    mb /= V;
+    for (int k = 0; k < nz; ++k)
+        for (int j = 0; j < ny; ++j)
+            for (int i = 0; i < nx; ++i) {
+                size_t c = IDX(i, j, k);
+                b[c] -= mb; x[c] = 0.0; d[c] = b[c];
+            }
+    const double bb = wdot(st, b, b);
+    double rr = bb;
+    int it = 0;
+    const int itmax = 200000;
+    while (bb > 0.0 && rr > 1e-28 * bb && it < itmax) {
+        varcoef_apply(st, d, q);
+        const double alpha = rr / wdot(st, d, q);
+#pragma omp parallel for
+        for (int k = 0; k < nz; ++k)
+            for (int j = 0; j < ny; ++j)
+                for (int i = 0; i < nx; ++i) {
+                    size_t c = IDX(i, j, k);
+                    x[c] += alpha * d[c];
+                    b[c] -= alpha * q[c];
+                }
+        const double rn = wdot(st, b, b);
+        const double beta = rn / rr;
+#pragma omp parallel for
+        for (int k = 0; k < nz; ++k)
+            for (int j = 0; j < ny; ++j)
+                for (int i = 0; i < nx; ++i) {
+                    size_t c = IDX(i, j, k);
+                    d[c] = b[c] + beta * d[c];
+                }
+        rr = rn;
+        ++it;
+    }
+    double mx = 0.0;
+    for (int k = 0; k < nz; ++k)
+        for (int j = 0; j < ny; ++j)
+            for (int i = 0; i < nx; ++i) mx += DZF(k) * x[IDX(i, j, k)];
+    mx /= V;
+    for (int k = 0; k < nz; ++k)
+        for (int j = 0; j < ny; ++j)
+            for (int i = 0; i < nx; ++i) x[IDX(i, j, k)] -= mx;
+    free(d); free(q);
+    return it;
+}
+
+void orc_set_solver(orc_state *st, int solver) { st->solver = solver ? 1 : 0; }
+
+/* rhs, p: N interior doubles; density from the CURRENT phase field */
+int orc_varcoef_solve(orc_state *st, const double *rhs, double *p)
+{
+    double *b = palloc(st), *x = palloc(st);
+    property_map(st, st->phi);
+    put_interior(st, b, rhs);
+    const int it = varcoef_solve(st, b, x);
+    get_interior(st, x, p);
+    free(b); free(x);
+    return it;
+}
+
 static const double RK_GAMMA[3] = {8.0 / 15.0, 5.0 / 12.0, 3.0 / 4.0};
 static const double RK_ZETA[3] = {0.0, -17.0 / 60.0, -5.0 / 12.0};
 
@@ -808,6 +928,35 @@ int orc_substep(orc_state *st, int stage, double dt)
                 st->hw[c] = st->rw[c];
             }
     fill_velocity_ghosts(st, st->us, st->vs, st->ws);
+
+    if (st->solver == 1) {
+        /* S4', S5': D((1/rho_f) d p_new) = D(u*)/(as dt);  u = u* - as dt (1/rho_f) d p_new */
+        const double *rho = st->rho;
+#pragma omp parallel for
+        for (int k = 0; k < nz; ++k)
+            for (int j = 0; j < ny; ++j)
+                for (int i = 0; i < nx; ++i) {
+                    size_t c = IDX(i, j, k);
+                    st->prhs[c] = ((st->us[c] - st->us[IDX(i - 1, j, k)]) / dx + (st->vs[c] - st->vs[IDX(i, j - 1, k)]) / dy +
+                                   (st->ws[c] - st->ws[IDX(i, j, k - 1)]) / DZF(k)) / (as * dt);
+                }
+        varcoef_solve(st, st->prhs, st->pnew);
+        fill_ghosts(st, st->pnew, BC_EVEN, 0, 0);
+        const double *pn = st->pnew;
+#pragma omp parallel for
+        for (int k = 0; k < nz; ++k)
+            for (int j = 0; j < ny; ++j)
+                for (int i = 0; i < nx; ++i) {
+                    size_t c = IDX(i, j, k), xp = IDX(i + 1, j, k), yp = IDX(i, j + 1, k), zp = IDX(i, j, k + 1);
+                    st->u[c] = st->us[c] - as * dt * (pn[xp] - pn[c]) / dx / (0.5 * (rho[c] + rho[xp]));
+                    st->v[c] = st->vs[c] - as * dt * (pn[yp] - pn[c]) / dy / (0.5 * (rho[c] + rho[yp]));
+                    st->w[c] = (k < kzf) ? st->ws[c] - as * dt * (pn[zp] - pn[c]) / DZC(k) / (0.5 * (rho[c] + rho[zp])) : 0.0;
+                }
+        fill_velocity_ghosts(st, st->u, st->v, st->w);
+        memcpy(st->pp, st->p, st->NP * sizeof(double));
+        memcpy(st->p, st->pnew, st->NP * sizeof(double));
+        return 0;
+    }
 
     /* S4: p_hat = 2p - p_prev (N7);  b = D((1 - rho0/rho_f) d p_hat) + rho0/(as dt) D(u*) */
     const double rho0 = fmin(P->rho1, P->rho2);

@@ -64,6 +64,14 @@ int orc_substep(orc_state *st, int stage, double dt);
 /* solves Lap p = rhs with the state's grid and z boundary condition; gauge: N17 */
 void orc_poisson_solve(orc_state *st, const double *rhs, double *p);
 
+/* SURVEY.md 8(f)-4 (the variable-coefficient alternative to the splitting): solver = 1 makes orc_substep solve
+ * D((1/rho_f) d p_new) = D(u*)/(a dt) and correct with u = u* - a dt (1/rho_f) d p_new (no p_hat anywhere); plain CG in the
+ * dzf-weighted inner product to a relative residual of 1e-14.  orc_varcoef_solve: that solve alone, density from the current
+ * phase field; returns the iterations.  Pinned against oracle/varcoef.py (sparse direct) and, for rho1 = rho2, against the
+ * splitting itself. */
+void orc_set_solver(orc_state *st, int solver);
+int orc_varcoef_solve(orc_state *st, const double *rhs, double *p);
+
 double orc_gamma(const orc_state *st);
 
 /* intermediates of the LAST substep (unpadded nx*ny*nz copies). names:

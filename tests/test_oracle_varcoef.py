@@ -141,3 +141,54 @@ def test_manufactured_solution_second_order():
         errs.append(np.abs(p - ex).max())
     orders = [np.log(errs[q] / errs[q + 1]) / np.log(sizes[q + 1] / sizes[q]) for q in range(3)]
     assert orders[2] > 1.8 and orders[1] > 1.7, (errs, orders)
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# the plain-C oracle's own variable-coefficient path (orc_varcoef_solve, orc_substep with solver = 1)
+
+@pytest.mark.parametrize("index,grid", [(0, (16, 16, 12)), (2, (16, 16, 12)), (4, (16, 8, 12))])
+def test_c_oracle_cg_solve_matches_the_sparse_direct_solve(oracle_mod, index, grid):
+    """Unpreconditioned CG in C (an iteration) against the bordered sparse direct solve (the definition): periodic ratio
+    10, walls ratio 1000, stretched walls ratio 10."""
+    cfg, f, dt, _ = W.make(index, grid=grid, ndrops=1, radius=0.2 if index else None)
+    o = oracle_mod.Oracle(cfg)
+    o.set_fields(**f)
+    rhs = np.random.default_rng(9).standard_normal(o.shape)
+    pc = o.varcoef_solve(rhs)
+    pd = V.solve(cfg, f["phi"], rhs)
+    assert np.abs(pc - pd).max() <= 1e-9 * np.abs(pd).max(), o.varcoef_iterations
+    o.close()
+
+
+def test_substep_with_the_variable_coefficient_solver_equals_the_splitting_for_matched_densities(oracle_mod):
+    """rho1 = rho2: the splitting is exact (its p_hat terms vanish), so both pressure paths give the same step."""
+    cfg, f, dt, _ = W.make(1, grid=(16, 16, 16), ndrops=1)
+    a, b = oracle_mod.Oracle(cfg), oracle_mod.Oracle(cfg)
+    b.set_solver(1)
+    for o in (a, b):
+        o.set_fields(**f)
+        o.step(dt)
+    fa, fb = a.get_fields(), b.get_fields()
+    for k in fa:
+        m = np.abs(fa[k]).max()
+        assert np.abs(fa[k] - fb[k]).max() <= 1e-10 * max(m, 1e-300), k
+    a.close(); b.close()
+
+
+def test_substep_with_the_variable_coefficient_solver_projects_exactly_at_ratio_1000(oracle_mod):
+    """D(u) after the correction = (residual of the solve) * a dt: divergence-free to the CG tolerance, walls, ratio 1000;
+    and the step differs from the splitting's (which extrapolates p_hat) only at the order of the splitting error."""
+    cfg, f, dt, _ = W.make(2, grid=(16, 16, 16), ndrops=1, radius=0.2)
+    o = oracle_mod.Oracle(cfg)
+    o.set_solver(1)
+    o.set_fields(**f)
+    for s in range(3):
+        o.substep(s, dt)
+    u = o.get_fields()
+    dx = cfg["lx"] / cfg["nx"]
+    div = (u["u"] - np.roll(u["u"], 1, 2)) / dx + (u["v"] - np.roll(u["v"], 1, 1)) / dx
+    wz = np.concatenate([np.zeros((1,) + u["w"].shape[1:]), u["w"]])[:-1]          # w below the first cell: the wall
+    div += (u["w"] - wz) / (cfg["lz"] / cfg["nz"])
+    umax = max(np.abs(u[k]).max() for k in "uvw")
+    assert np.abs(div).max() * dx / max(umax, 1.0) <= 1e-10
+    o.close()

@@ -300,6 +300,8 @@ def main():
     ap.add_argument("--no-cufft", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--pressure-solver", type=int, default=0, choices=[0, 1],
+                    help="1: the RK3 step with the variable-coefficient multigrid pressure path (SURVEY 8(f)-4; rtol 1e-10) instead of the splitting")
     ap.add_argument("--varcoef", action="store_true", help="time fizzy_poisson_solve_varcoef (SURVEY 8(f)-4) instead of the RK3 step")
     args = ap.parse_args()
     if args.varcoef:
@@ -337,6 +339,8 @@ def main():
     cfg, f, dt, _ = W.make(args.workload, grid=tuple(args.grid) if args.grid else None)
     cells = cfg["nx"] * cfg["ny"] * cfg["nz"]
     fz = Fizzy(cfg, device="cuda:%d" % local_rank)
+    if args.pressure_solver:
+        fz.fizzy_set_pressure_solver(1, rtol=1e-10, max_iter=200)
     names = ["u", "v", "w", "p", "phi"] + (["T"] if cfg["heat"] else [])
     dev = {k: torch.from_numpy(f[k]).to("cuda:%d" % local_rank) for k in names}
     fz.fizzy_set_fields(**dev)
@@ -456,6 +460,7 @@ def main():
             "config": {"workload": cfg["name"], "grid": [cfg["nx"], cfg["ny"], cfg["nz"]], "dt": dt,
                        "cache": "inputs larger than L2 (each field %.0f MB, 126 MB L2)" % (cells * 8 / 1e6),
                        "parallelism": "replicas x%d" % world, "finite": finite,
+                       "pressure_solver": "variable-coefficient multigrid CG, rtol 1e-10" if args.pressure_solver else "splitting + FFT/tridiagonal",
                        "byte_model": "SURVEY.md 8(d): %.0f B/cell/substep, every substep counted in full (stage 0 reads no RK "
                                      "history and stage 2 writes none: those discounts are NOT taken)" % substep_model_bytes(cfg),
                        "timing": "value: CUDA events on the library stream, per-kernel timing off; kernel table: second pass of "

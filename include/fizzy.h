@@ -161,6 +161,17 @@ fizzy_status fizzy_poisson_solve(fizzy_ctx *ctx, const double *rhs, double *p);
  * FIZZY_EINVAL: NULL rhs / p / dev_work, rtol <= 0, max_iter < 1, misaligned dev_work.  FIZZY_ENOMEM: work_bytes too small.
  * FIZZY_ESTATE: phi == NULL before fizzy_set_fields.  Not converged within max_iter is NOT an error: check *relres. */
 size_t fizzy_varcoef_workspace_bytes(const fizzy_ctx *ctx);
+
+/* Choose the pressure path of fizzy_rk3_substep (PAPER.md:36 offers both):
+ *   solver 0 (default): the constant-coefficient splitting, direct FFT / tridiagonal solve (BASELINE.json:5(iv),(v));
+ *   solver 1: the variable-coefficient problem  D((1/rho_f) d p_new) = D(u*)/(a dt)  by the multigrid-preconditioned CG above
+ *             (to rtol, at most max_iter iterations), then  u = u* - a dt (1/rho_f) d p_new;  no extrapolated pressure, no
+ *             reference density.  dev_work: caller-owned DEVICE scratch of fizzy_varcoef_workspace_bytes(ctx) bytes, 256-byte
+ *             aligned, which must stay valid while solver 1 is selected.  Every substep then synchronises the stream, CUDA
+ *             graph replay is bypassed, and a solve that misses rtol within max_iter makes the substep return FIZZY_ECUDA.
+ * Only between RK3 steps (FIZZY_ESTATE otherwise).  FIZZY_EINVAL / FIZZY_ENOMEM as for fizzy_poisson_solve_varcoef. */
+fizzy_status fizzy_set_pressure_solver(fizzy_ctx *ctx, int solver, void *dev_work, size_t work_bytes, double rtol,
+                                       int max_iter);
 fizzy_status fizzy_poisson_solve_varcoef(fizzy_ctx *ctx, const double *rhs, const double *phi, double *p,
                                          void *dev_work, size_t work_bytes, double rtol, int max_iter,
                                          int *iters, double *relres);

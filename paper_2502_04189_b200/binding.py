@@ -20,7 +20,7 @@ EXPORTS = ["fizzy_workspace_bytes", "fizzy_create", "fizzy_destroy", "fizzy_set_
            "fizzy_rk3_substep", "fizzy_poisson_solve", "fizzy_get_fields", "fizzy_gamma", "fizzy_diagnostics",
            "fizzy_launch_count", "fizzy_last_error", "fizzy_timing_enable", "fizzy_timing_get",
            "fizzy_rk3_step", "fizzy_graph_enable", "fizzy_stable_dt", "fizzy_check_finite",
-           "fizzy_varcoef_workspace_bytes", "fizzy_poisson_solve_varcoef"]
+           "fizzy_varcoef_workspace_bytes", "fizzy_poisson_solve_varcoef", "fizzy_set_pressure_solver"]
 
 
 class FizzyGrid(C.Structure):
@@ -74,6 +74,8 @@ def load_library(path: str = LIB_PATH) -> C.CDLL:
     lib.fizzy_poisson_solve_varcoef.restype = C.c_int
     lib.fizzy_poisson_solve_varcoef.argtypes = [vp, dp, dp, dp, vp, C.c_size_t, C.c_double, C.c_int,
                                                 C.POINTER(C.c_int), C.POINTER(C.c_double)]
+    lib.fizzy_set_pressure_solver.restype = C.c_int
+    lib.fizzy_set_pressure_solver.argtypes = [vp, C.c_int, vp, C.c_size_t, C.c_double, C.c_int]
     lib.fizzy_diagnostics.restype = C.c_int
     lib.fizzy_diagnostics.argtypes = [vp, C.POINTER(C.c_double)]
     lib.fizzy_rk3_step.restype = C.c_int
@@ -218,6 +220,17 @@ class Fizzy:
                                                          self._vc_work.data_ptr(), nbytes, float(rtol), int(max_iter),
                                                          C.byref(it), C.byref(rr)))
         return it.value, rr.value
+
+    def fizzy_set_pressure_solver(self, solver: int, rtol=1e-12, max_iter=200):
+        """solver 1 = the variable-coefficient multigrid path; the scratch tensor is torch-owned and kept alive here."""
+        with self._on_device():
+            ptr, nbytes = None, 0
+            if solver == 1:
+                nbytes = _lib.fizzy_varcoef_workspace_bytes(self._h)
+                if getattr(self, "_ps_work", None) is None or self._ps_work.numel() < nbytes:
+                    self._ps_work = self._torch.empty(nbytes, dtype=self._torch.uint8, device=self.device)
+                ptr = self._ps_work.data_ptr()
+            self._check(_lib.fizzy_set_pressure_solver(self._h, int(solver), ptr, nbytes, float(rtol), int(max_iter)))
 
     def fizzy_diagnostics(self) -> np.ndarray:
         out = (C.c_double * 8)()

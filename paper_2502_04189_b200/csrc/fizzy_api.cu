@@ -87,6 +87,13 @@ struct fizzy_ctx {
     // still hold the velocity of the stage start and corr_coef = a dt / rho0 of the pending correction
     bool corr_pending = false;
     double corr_coef = 0.0;
+    // pressure path of the substep: 0 = the constant-coefficient splitting (FFT solver), 1 = the variable-coefficient problem
+    // by multigrid-preconditioned CG, with the caller's scratch (fizzy_set_pressure_solver)
+    int solver = 0;
+    void *mg_work = nullptr;
+    size_t mg_bytes = 0;
+    double mg_rtol = 1e-12;
+    int mg_maxit = 200;
     long long launches;
     std::string err;
 };
@@ -663,10 +670,35 @@ extern "C" fizzy_status fizzy_rk3_substep(fizzy_ctx *c, int stage, double dt)
     A.u = c->u; A.v = c->v; A.w = c->w; A.phi = c->phi; A.kappa = c->kappa;
     A.rnx = c->rnx; A.rny = c->rny; A.rnz = c->rnz; A.p = c->p; A.pp = c->pp; A.phat = c->phat; A.T = c->T;
     A.us = c->us; A.vs = c->vs; A.ws = c->ws; A.hu = c->hu; A.hv = c->hv; A.hw = c->hw;
-    A.scal = c->scal; A.dt = dt; A.gs = gs; A.zs = zs; A.adt = as * dt; A.keep_h = stage != 2;
+    A.scal = c->scal; A.dt = dt; A.gs = gs; A.zs = zs; A.keep_h = stage != 2;
+    A.adt = c->solver == 1 ? 0.0 : as * dt;   // the p_hat part of the splitting rides in the predictor (D2); none with solver 1
     FZ_TB(FZK_MOM);
     FZ_CUDA(launch_momentum(c, grid, block, &A));
     FZ_LAUNCHED(FZK_MOM);
+    if (c->solver == 1) {
+        // S4', S5': D((1/rho_f) d p_new) = D(u*)/(a dt) by multigrid-preconditioned CG, then
+        // u = u* - a dt (1/rho_f) d p_new.  No p_hat, no deferred correction; the solve synchronises the stream.
+        FZ_TB(FZK_OTHER);
+        k_div_rhs<<<grid, block, 0, c->stream>>>(P, c->us, c->vs, c->ws, 1.0 / (as * dt), c->pn);
+        FZ_LAUNCHED(FZK_OTHER);
+        int iters = 0;
+        double relres = 0.0;
+        s = fizzy_poisson_solve_varcoef(c, c->pn, nullptr, c->pn, c->mg_work, c->mg_bytes, c->mg_rtol, c->mg_maxit, &iters, &relres);
+        if (s != FIZZY_OK) return s;
+        if (!(relres <= c->mg_rtol)) return fail(c, FIZZY_ECUDA, "fizzy_rk3_substep: the variable-coefficient pressure solve did not reach rtol within max_iter");
+        FZ_TB(FZK_CORRECT);
+        if (stage == 2)
+            k_correct_var<true><<<grid, block, 0, c->stream>>>(P, c->us, c->vs, c->ws, c->pn, c->phi, c->u, c->v, c->w, as * dt, c->scal);
+        else
+            k_correct_var<false><<<grid, block, 0, c->stream>>>(P, c->us, c->vs, c->ws, c->pn, c->phi, c->u, c->v, c->w, as * dt, c->scal);
+        FZ_LAUNCHED(FZK_CORRECT);
+        double *old = c->pp;
+        c->pp = c->p;
+        c->p = c->pn;
+        c->pn = old;
+        c->next_stage = (stage + 1) % 3;
+        return FIZZY_OK;
+    }
     // S4: b = rho0/(a dt) D(u**), FFT x (fused), FFT y, tridiagonal z, inverse
     FZ_TB(FZK_FFTX_FWD);
     FZ_CUDA(fz_fftx_launch(0, c->log2nx, P, nullptr, c->us, c->vs, c->ws, P.rho0 / (as * dt), c->spec, nullptr,
@@ -795,7 +827,7 @@ extern "C" fizzy_status fizzy_rk3_step(fizzy_ctx *c, double dt)
     if (!c->fields_set) return fail(c, FIZZY_ESTATE, "fizzy_set_fields has not been called");
     if (c->next_stage != 0) return fail(c, FIZZY_ESTATE, "fizzy_rk3_step must start at stage 0");
     fizzy_status s = FIZZY_OK;
-    if (!c->graph_on || c->timing) {   // plain launches (per-kernel events cannot be recorded into a replayed graph)
+    if (!c->graph_on || c->timing || c->solver == 1) {   // plain launches (per-kernel events cannot be recorded into a replayed graph)
         for (int stage = 0; stage < 3 && s == FIZZY_OK; ++stage) s = fizzy_rk3_substep(c, stage, dt);
         return s;
     }
@@ -868,6 +900,24 @@ void mg_grid(const FzMgLevel &L, dim3 &grid, dim3 &block)
 }
 
 }  // namespace
+
+extern "C" fizzy_status fizzy_set_pressure_solver(fizzy_ctx *c, int solver, void *dev_work, size_t work_bytes, double rtol,
+                                                  int max_iter)
+{
+    if (!c) return FIZZY_EINVAL;
+    FZ_DEVICE();
+    if (solver != 0 && solver != 1) return fail(c, FIZZY_EINVAL, "solver must be 0 (splitting) or 1 (variable-coefficient multigrid)");
+    FZ_FLUSH();
+    if (c->next_stage != 0) return fail(c, FIZZY_ESTATE, "the pressure solver can only be changed between RK3 steps");
+    if (solver == 1) {
+        if (!dev_work || (reinterpret_cast<uintptr_t>(dev_work) & 255) || !(rtol > 0.0) || max_iter < 1)
+            return fail(c, FIZZY_EINVAL, "solver 1 needs 256-byte aligned dev_work, rtol > 0, max_iter >= 1");
+        if (work_bytes < mg_plan(c).doubles * sizeof(double)) return fail(c, FIZZY_ENOMEM, "dev_work is smaller than fizzy_varcoef_workspace_bytes");
+        c->mg_work = dev_work; c->mg_bytes = work_bytes; c->mg_rtol = rtol; c->mg_maxit = max_iter;
+    }
+    c->solver = solver;
+    return FIZZY_OK;
+}
 
 extern "C" size_t fizzy_varcoef_workspace_bytes(const fizzy_ctx *c)
 {

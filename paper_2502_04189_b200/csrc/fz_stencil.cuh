@@ -292,6 +292,48 @@ __global__ void k_correct(FzP P, const double *__restrict__ us, const double *__
     }
 }
 
+// ---------------------------------------------------------------- S4', S5': the variable-coefficient path
+// rhs = coef D(u*)   (coef = 1/(a dt); the velocity below the first cell of a wall-bounded grid is the wall: 0)
+__global__ void k_div_rhs(FzP P, const double *__restrict__ us, const double *__restrict__ vs,
+                          const double *__restrict__ ws, double coef, double *__restrict__ rhs)
+{
+    FZ_CELL_IJK
+    const FzZ z = fz_zn(P, k);
+    const unsigned nx = P.nx, sxy = (unsigned)P.sxy;
+    const unsigned pl = (unsigned)k * sxy, row = pl + nx * j, c = row + i;
+    const unsigned xm = row + fz_im(i, P.nx), ym = pl + nx * fz_im(j, P.ny) + i, zm = (unsigned)z.km * sxy + nx * j + i;
+    const double wl = z.gm ? 0.0 : ws[zm];
+    rhs[c] = coef * ((us[c] - us[xm]) * P.idx + (vs[c] - vs[ym]) * P.idy + (ws[c] - wl) * P.idzf[k]);
+}
+
+// u = u* - a dt (1/rho_f) d_a p_new,  rho_f = 1/2 (rho + rho(+1_a)) of phi_new (N11); max|u| at stage 2
+template <bool WITH_MAX>
+__global__ void k_correct_var(FzP P, const double *__restrict__ us, const double *__restrict__ vs,
+                              const double *__restrict__ ws, const double *__restrict__ pn,
+                              const double *__restrict__ phi, double *__restrict__ u, double *__restrict__ v,
+                              double *__restrict__ w, double adt, double *umax)
+{
+    FZ_CELL_IJK
+    const FzZ z = fz_zn(P, k);
+    const unsigned nx = P.nx, sxy = (unsigned)P.sxy;
+    const unsigned pl = (unsigned)k * sxy, row = pl + nx * j, c = row + i;
+    const unsigned xp = row + fz_ip(i, P.nx), yp = pl + nx * fz_ip(j, P.ny) + i, zp = (unsigned)z.kp * sxy + nx * j + i;
+    const double p0 = pn[c], r0 = P.rho2 + P.drho * fz_clip01(phi[c]);
+    const double un = us[c] - adt * (pn[xp] - p0) * P.idx / (0.5 * (r0 + P.rho2 + P.drho * fz_clip01(phi[xp])));
+    const double vn = vs[c] - adt * (pn[yp] - p0) * P.idy / (0.5 * (r0 + P.rho2 + P.drho * fz_clip01(phi[yp])));
+    double wn = 0.0;
+    if (k < P.kzf) wn = ws[c] - adt * (pn[zp] - p0) * P.idzc[k] / (0.5 * (r0 + P.rho2 + P.drho * fz_clip01(phi[zp])));
+    u[c] = un;
+    v[c] = vn;
+    w[c] = wn;
+    if (WITH_MAX) {
+        double m = fmax(fabs(un), fmax(fabs(vn), fabs(wn)));
+        for (int o = 16; o > 0; o >>= 1) m = fmax(m, __shfl_xor_sync(0xffffffffu, m, o));
+        if (((threadIdx.x + blockDim.x * threadIdx.y) & 31) == 0 && m > *reinterpret_cast<volatile double *>(umax))
+            fz_atomic_max_nonneg(umax, m);
+    }
+}
+
 // p_hat = 2p - p_prev (N7) of freshly loaded pressures
 __global__ void k_phat(FzP P, const double *__restrict__ p, const double *__restrict__ pp, double *__restrict__ phat)
 {

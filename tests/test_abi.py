@@ -93,3 +93,17 @@ def test_product_does_not_import_the_oracle():
                 text = open(os.path.join(dirpath, fn)).read()
                 assert not re.search(r"^\s*(from|import)\s+oracle\b", text, flags=re.M), fn
                 assert "fizzy_oracle" not in text and "liborc" not in text, fn
+
+
+def test_variable_coefficient_entry_points_reject_null_contexts(binding):
+    """SURVEY.md 8(f)-4 calls: argument errors come back as status codes without a GPU."""
+    lib = C.CDLL(binding.LIB_PATH)
+    lib.fizzy_varcoef_workspace_bytes.restype = C.c_size_t
+    lib.fizzy_varcoef_workspace_bytes.argtypes = [C.c_void_p]
+    assert lib.fizzy_varcoef_workspace_bytes(None) == 0
+    lib.fizzy_poisson_solve_varcoef.restype = C.c_int
+    lib.fizzy_poisson_solve_varcoef.argtypes = [C.c_void_p] * 5 + [C.c_size_t, C.c_double, C.c_int, C.c_void_p, C.c_void_p]
+    assert lib.fizzy_poisson_solve_varcoef(None, None, None, None, None, 0, 1e-10, 10, None, None) == binding.FIZZY_EINVAL
+    lib.fizzy_set_pressure_solver.restype = C.c_int
+    lib.fizzy_set_pressure_solver.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_size_t, C.c_double, C.c_int]
+    assert lib.fizzy_set_pressure_solver(None, 1, None, 0, 1e-10, 10) == binding.FIZZY_EINVAL

@@ -297,19 +297,21 @@ k_momentum_march(FzP P, FzMomArgs A, int KC)
         // RK histories: loaded one plane ahead (registers), so their latency hides behind a whole plane
         const double hu_old = hu_nx, hv_old = hv_nx, hw_old = hw_nx;
         if (use_h && k + 1 < k1) { hu_nx = A.hu[c + sxy]; hv_nx = A.hv[c + sxy]; hw_nx = A.hw[c + sxy]; }
-        // ghost rules at the walls: the ring slot of plane -1 / nz arrives holding the mirrored interior plane; the two
-        // plane steps that read it turn it into the ghost plane first (no-slip: -u, -v; impermeable: w = 0, R_z = 0; phi,
-        // kappa, p_hat, T are even and stay), so that the other nz-2 steps -- and every step of a periodic grid -- carry no
-        // sign factors (round 2: nine DMUL and a dozen select / predicate instructions per cell, in every configuration)
-        if (P.z_wall && (k == 0 || k == P.nz - 1)) {
+        // ghost rules at the walls: the ring slot of plane -1 / nz arrives holding the mirrored interior plane.
+        // rho1 == rho2 (GHOST_SMEM): the two plane steps that read it turn it into the ghost plane first (no-slip: -u, -v;
+        // impermeable: w = 0; phi, kappa, T are even and stay), so that the other nz-2 steps -- and every step of a periodic
+        // grid -- carry no sign factors (round 2: nine DMUL and a dozen select / predicate instructions per cell, in every
+        // configuration).  rho1 != rho2: the factors are applied when a ghost plane is READ, as before -- with nine staged
+        // fields at 128 registers the extra block costs that variant 3-4 % (measured on configs 3 and 5).
+        constexpr bool GHOST_SMEM = !VARRHO;
+        const bool gm = !GHOST_SMEM && P.z_wall && k == 0, gp = !GHOST_SMEM && P.z_wall && k == P.nz - 1;
+        const double sgm = gm ? -1.0 : 1.0, sgp = gp ? -1.0 : 1.0, wm = gm ? 0.0 : 1.0;
+        if (GHOST_SMEM && P.z_wall && (k == 0 || k == P.nz - 1)) {
             const int gb = (k == 0 ? om : op) - cidx;
             for (int e = t; e < MPS; e += MTX * MTY) {
                 smm[F::U * (MRING * MPS) + gb + e] = -smm[F::U * (MRING * MPS) + gb + e];
                 smm[F::V * (MRING * MPS) + gb + e] = -smm[F::V * (MRING * MPS) + gb + e];
-                if (k == 0) {
-                    smm[F::W * (MRING * MPS) + gb + e] = 0.0;
-                    if (VARRHO) smm[F::RZ * (MRING * MPS) + gb + e] = 0.0;
-                }
+                if (k == 0) smm[F::W * (MRING * MPS) + gb + e] = 0.0;
             }
             __syncthreads();
         }
@@ -322,13 +324,13 @@ k_momentum_march(FzP P, FzMomArgs A, int KC)
         const double izfp = izf_p;   // 1/dzf[k+1]
         const double u000 = S_(F::U, 0, 0, o0), up00 = S_(F::U, 1, 0, o0), um00 = S_(F::U, -1, 0, o0);
         const double u0p0 = S_(F::U, 0, 1, o0), u0m0 = S_(F::U, 0, -1, o0), ump0 = S_(F::U, -1, 1, o0);
-        const double u00p = S_(F::U, 0, 0, op), u00m = S_(F::U, 0, 0, om), um0p = S_(F::U, -1, 0, op);
+        const double u00p = sgp * S_(F::U, 0, 0, op), u00m = sgm * S_(F::U, 0, 0, om), um0p = sgp * S_(F::U, -1, 0, op);
         const double v000 = S_(F::V, 0, 0, o0), vp00 = S_(F::V, 1, 0, o0), vm00 = S_(F::V, -1, 0, o0);
         const double v0p0 = S_(F::V, 0, 1, o0), v0m0 = S_(F::V, 0, -1, o0), vpm0 = S_(F::V, 1, -1, o0);
-        const double v00p = S_(F::V, 0, 0, op), v00m = S_(F::V, 0, 0, om), v0mp = S_(F::V, 0, -1, op);
+        const double v00p = sgp * S_(F::V, 0, 0, op), v00m = sgm * S_(F::V, 0, 0, om), v0mp = sgp * S_(F::V, 0, -1, op);
         const double w000 = S_(F::W, 0, 0, o0), wp00 = S_(F::W, 1, 0, o0), wm00 = S_(F::W, -1, 0, o0);
         const double w0p0 = S_(F::W, 0, 1, o0), w0m0 = S_(F::W, 0, -1, o0);
-        const double w00m = S_(F::W, 0, 0, om), wp0m = S_(F::W, 1, 0, om), w0pm = S_(F::W, 0, 1, om);
+        const double w00m = wm * S_(F::W, 0, 0, om), wp0m = wm * S_(F::W, 1, 0, om), w0pm = wm * S_(F::W, 0, 1, om);
         const double f000 = S_(F::PHI, 0, 0, o0), fp00 = S_(F::PHI, 1, 0, o0), f0p0 = S_(F::PHI, 0, 1, o0),
                      f00p = S_(F::PHI, 0, 0, op);
         double m000, mp00, mm00, m0p0, m0m0, m00p, m00m, mpp0, mpm0, mmp0, mp0p, mp0m, mm0p, m0pp, m0pm, m0mp;
@@ -396,7 +398,7 @@ k_momentum_march(FzP P, FzMomArgs A, int KC)
             double M = 0.0;
             if (VARRHO) {
                 const double Rty = 0.25 * (S_(F::RY, 0, 0, o0) + S_(F::RY, 1, 0, o0) + S_(F::RY, 0, -1, o0) + S_(F::RY, 1, -1, o0));
-                const double Rtz = 0.25 * (S_(F::RZ, 0, 0, o0) + S_(F::RZ, 1, 0, o0) + S_(F::RZ, 0, 0, om) + S_(F::RZ, 1, 0, om));
+                const double Rtz = 0.25 * (S_(F::RZ, 0, 0, o0) + S_(F::RZ, 1, 0, o0) + wm * (S_(F::RZ, 0, 0, om) + S_(F::RZ, 1, 0, om)));
                 M = P.drho * Gam * (S_(F::RX, 0, 0, o0) * (up00 - um00) * (0.5 * dx) + Rty * (u0p0 - u0m0) * (0.5 * dy) +
                                     Rtz * (u00p - u00m) * P.igz[k]);
             }
@@ -424,7 +426,7 @@ k_momentum_march(FzP P, FzMomArgs A, int KC)
             double M = 0.0;
             if (VARRHO) {
                 const double Rtx = 0.25 * (S_(F::RX, 0, 0, o0) + S_(F::RX, 0, 1, o0) + S_(F::RX, -1, 0, o0) + S_(F::RX, -1, 1, o0));
-                const double Rtz = 0.25 * (S_(F::RZ, 0, 0, o0) + S_(F::RZ, 0, 1, o0) + S_(F::RZ, 0, 0, om) + S_(F::RZ, 0, 1, om));
+                const double Rtz = 0.25 * (S_(F::RZ, 0, 0, o0) + S_(F::RZ, 0, 1, o0) + wm * (S_(F::RZ, 0, 0, om) + S_(F::RZ, 0, 1, om)));
                 M = P.drho * Gam * (S_(F::RY, 0, 0, o0) * (v0p0 - v0m0) * (0.5 * dy) + Rtx * (vp00 - vm00) * (0.5 * dx) +
                                     Rtz * (v00p - v00m) * P.igz[k]);
             }

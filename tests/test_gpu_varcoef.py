@@ -12,7 +12,7 @@ pytestmark = pytest.mark.gpu
 CASES = {
     "periodic_ratio10_32x16x24": lambda: W.make(0, grid=(32, 16, 24)),
     "walls_ratio1000_32x32x16": lambda: W.make(2, grid=(32, 32, 16), ndrops=1, radius=0.2),
-    "stretched_walls_ratio10_64x32x24": lambda: W.make(4, grid=(64, 32, 24), ndrops=2, radius=0.3),
+    "stretched_walls_ratio10_32x16x24": lambda: W.make(4, grid=(32, 16, 24), ndrops=1, radius=0.3),
     "odd_nz_single_level_32x32x15": lambda: W.make(2, grid=(32, 32, 15), ndrops=1, radius=0.2),
     "two_levels_nz12_32x64x12": lambda: W.make(0, grid=(32, 64, 12)),
 }

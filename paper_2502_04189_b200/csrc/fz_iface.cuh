@@ -123,8 +123,10 @@ k_iface_march(FzP P, const double *__restrict__ psi, const double *__restrict__ 
     double nz0 = 0.0, nzp = 0.0, nfz_prev = 0.0, Rz_prev = 0.0;
     const unsigned gc = (unsigned)((i0 + tx) + P.nx * (j0 + ty));
     double igz_n = P.igz[k0 - 2], idzc_n = 0.0, idzf_n = 0.0;   // z metrics: loaded one step ahead (plane k0-3 is never used)
-    auto step = [&](auto Sc, int kk) {
-        constexpr int S = decltype(Sc)::value;
+    // PH = 0, 1, 2: the first three steps of a chunk (r only | + half normals | + the z face below the first plane); PH = 3:
+    // a full step.  A compile-time phase keeps the three prologue tests out of the steady-state steps.
+    auto step = [&](auto Sc, auto Pc, int kk) {
+        constexpr int S = decltype(Sc)::value, PH = decltype(Pc)::value;
         constexpr int om = ((S + IRING - 1) % IRING) * IPS, o0 = (S % IRING) * IPS, op = ((S + 1) % IRING) * IPS;
         constexpr int rm = ((S + 2) % 3) * INS, r0s = (S % 3) * INS, rp = ((S + 1) % 3) * INS;   // r planes kk-1, kk, kk+1
         constexpr int n0 = (S % 2) * 2 * INS, nm = ((S + 1) % 2) * 2 * INS;                       // half-normal planes kk, kk-1
@@ -139,7 +141,7 @@ k_iface_march(FzP P, const double *__restrict__ psi, const double *__restrict__ 
         igz_n = P.igz[kk + 1];
         const double idzc_k = idzc_n, idzf_k = idzf_n;   // metrics of plane k = kk-1, loaded one step ago
         idzc_n = P.idzc[kk]; idzf_n = P.idzf[kk];
-        if (kk < k0 - 1) return;
+        if (PH < 1) return;
         {   // half normals of plane kk: own cell, then the halo cross
             double ax, ay, az;
             normal(PSIc, om, o0, op, igz, ax, ay, az);
@@ -151,14 +153,14 @@ k_iface_march(FzP P, const double *__restrict__ psi, const double *__restrict__ 
             }
         }
         const int k = kk - 1;
-        if (k < k0 - 1) return;
+        if (PH < 2) return;
         const double f0 = PHIc[om], r0 = RRc[rm];
         // z face k+1/2; the face k-1/2 is carried in registers.  On a wall face both terms vanish by themselves, exactly:
         // the ghost planes hold the mirrored psi and phi (and igz is mirrored), so nhat_z of the ghost cell is bit for bit
         // minus that of the wall cell (nf_z = 0, N3/walls) and phi(ghost) - phi(wall cell) = 0 (R_z = 0)
         const double nfzp = nz0 + nzp;
         const double Rzp = P.eps * (PHIc[o0] - f0) * idzc_k - fz_sharp2(r0, RRc[r0s]) * nfzp;
-        if (k < k0) { nfz_prev = nfzp; Rz_prev = Rzp; return; }
+        if (PH < 3) { nfz_prev = nfzp; Rz_prev = Rzp; return; }
         // half normals of plane k were written one step ago: visible after this step's barrier
         const double ax = NHXc[nm], ay = NHYc[nm];
         const double nfxp = ax + NHXc[nm + 1], nfxm = NHXc[nm - 1] + ax;
@@ -173,19 +175,25 @@ k_iface_march(FzP P, const double *__restrict__ psi, const double *__restrict__ 
         if (STORE_R) { rnx[c] = Rxp; rny[c] = Ryp; rnz[c] = Rzp; }
         nfz_prev = nfzp; Rz_prev = Rzp;
     };
-    // steps kk = k0-2 .. k1 (plane k = kk-1 = k1-1 is the last one written)
-    for (int kk = k0 - 2; kk <= k1; kk += IRING) {
-        step(std::integral_constant<int, 0>{}, kk);
+    // steps kk = k0-2 .. k1 (plane k = kk-1 = k1-1 is the last one written); a chunk holds at least one plane, so the three
+    // prologue steps always run
+#define IC_(n_) std::integral_constant<int, n_>{}
+    step(IC_(0), IC_(0), k0 - 2);
+    step(IC_(1), IC_(1), k0 - 1);
+    step(IC_(2), IC_(2), k0);
+    for (int kk = k0 + 1; kk <= k1; kk += IRING) {
+        step(IC_(3), IC_(3), kk);
         if (kk + 1 > k1) break;
-        step(std::integral_constant<int, 1>{}, kk + 1);
+        step(IC_(4), IC_(3), kk + 1);
         if (kk + 2 > k1) break;
-        step(std::integral_constant<int, 2>{}, kk + 2);
+        step(IC_(5), IC_(3), kk + 2);
         if (kk + 3 > k1) break;
-        step(std::integral_constant<int, 3>{}, kk + 3);
+        step(IC_(0), IC_(3), kk + 3);
         if (kk + 4 > k1) break;
-        step(std::integral_constant<int, 4>{}, kk + 4);
+        step(IC_(1), IC_(3), kk + 4);
         if (kk + 5 > k1) break;
-        step(std::integral_constant<int, 5>{}, kk + 5);
+        step(IC_(2), IC_(3), kk + 5);
     }
+#undef IC_
     fz_cp_async_wait<0>();
 }

@@ -35,7 +35,7 @@ sys.path.insert(0, ROOT)
 
 from paper_2502_04189_b200 import workloads as W  # noqa: E402
 
-TRAFFIC_CSV, TRAFFIC_MD = "r2d_traffic.csv", "r2d_ncu_full.md"
+TRAFFIC_CSV, TRAFFIC_MD = "r2e_traffic.csv", "r2e_ncu_full.md"
 METRIC = "fp64 Mcell-substeps/s per RK3 step"
 UNIT = "Mcell-substeps/s"
 

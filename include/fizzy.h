@@ -141,6 +141,36 @@ fizzy_status fizzy_stable_dt(fizzy_ctx *ctx, double cfl, double *dt);
 /* Number of non-finite values among u, v, w, p, phi (and T with heat on); one pass, synchronises the stream. */
 fizzy_status fizzy_check_finite(fizzy_ctx *ctx, long long *count);
 
+/* Count the non-finite values (Inf, NaN) in up to 8 fields WITHOUT a context, a workspace or any allocation: the health check
+ * of fizzy_check_finite (failure detection) for code that is handed field pointers and nothing else.
+ * Who needs this: a monitoring or output hook that the solver calls between steps with device pointers to u, v, w, p, phi, T.
+ * Such a hook owns no device memory and must not ask for any: the host application has usually given the whole GPU to its own
+ * pool allocator (a cudaMalloc from the hook fails, or takes memory the solver counted on), and cudaMalloc / cudaFree
+ * synchronise the device, which would stall the solver's streams in the middle of a run.  The same holds inside any loop
+ * where an implicit device-wide synchronisation is not acceptable.
+ * Scratch: a file-scope __device__ array inside libfizzy.so (256 KiB + 256 B on every GPU that loads the library, held until
+ * the process exits) -- one partial count per 4096-value chunk, which is what limits n:
+ *     n <= FIZZY_STATIC_MAX_VALUES = 2^27 values per field (a 512^3 grid), nfields <= FIZZY_STATIC_MAX_FIELDS = 8.
+ * Larger n is rejected with FIZZY_EINVAL and a message; nothing is launched.  The call makes no cudaMalloc, cudaFree or
+ * allocating library call.
+ * dev_fields: HOST array of nfields pointers, each to n doubles in memory of the CURRENT device (device or managed memory;
+ *             host pointers are rejected -- staging them would need an allocation).  The fields are only read.
+ * cuda_stream: cudaStream_t the work is enqueued on (NULL = default stream).  count: HOST pointer, receives the number of
+ * non-finite values over all fields.  Synchronises that stream (the count is read back), nothing else.
+ * err / err_len: optional HOST buffer for a message when the status is not FIZZY_OK (may be NULL / 0).
+ * First call on a device: it also looks up the device address of the built-in array on the current device
+ * (cudaGetSymbolAddress, once per device, which may load the library's GPU code there).  Make that first call during
+ * start-up, before any stream capture begins.
+ * Sharing: every call on a device uses the same array, and the array keeps the last call's contents.  The call clears the two
+ * words that must start at zero itself; calls that overlap on the GPU (two streams, two host threads) race on the array and
+ * return garbage -- issue them one after another.
+ * FIZZY_EINVAL: NULL dev_fields / count / field pointer, nfields or n out of range, a field that is not memory of the
+ * current device.  FIZZY_ECUDA: a CUDA runtime call failed (text in err). */
+#define FIZZY_STATIC_MAX_VALUES 134217728LL
+#define FIZZY_STATIC_MAX_FIELDS 8
+fizzy_status fizzy_count_nonfinite_static(const double *const *dev_fields, int nfields, long long n, void *cuda_stream,
+                                          long long *count, char *err, size_t err_len);
+
 /* Solve Lap p = rhs with the context's grid and z boundary condition (periodic x, y; periodic
  * or homogeneous Neumann z): FFT in x and y, tridiagonal in z (BASELINE.json:5(iv)).  The
  * singular mean mode follows N17: last row replaced by p_hat(nz-1) = 0, then the dzf-weighted

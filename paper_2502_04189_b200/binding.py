@@ -20,7 +20,8 @@ EXPORTS = ["fizzy_workspace_bytes", "fizzy_create", "fizzy_destroy", "fizzy_set_
            "fizzy_rk3_substep", "fizzy_poisson_solve", "fizzy_get_fields", "fizzy_gamma", "fizzy_diagnostics",
            "fizzy_launch_count", "fizzy_last_error", "fizzy_timing_enable", "fizzy_timing_get",
            "fizzy_rk3_step", "fizzy_graph_enable", "fizzy_stable_dt", "fizzy_check_finite",
-           "fizzy_varcoef_workspace_bytes", "fizzy_poisson_solve_varcoef", "fizzy_set_pressure_solver"]
+           "fizzy_varcoef_workspace_bytes", "fizzy_poisson_solve_varcoef", "fizzy_set_pressure_solver",
+           "fizzy_count_nonfinite_static"]
 
 
 class FizzyGrid(C.Structure):
@@ -86,6 +87,9 @@ def load_library(path: str = LIB_PATH) -> C.CDLL:
     lib.fizzy_stable_dt.argtypes = [vp, C.c_double, C.POINTER(C.c_double)]
     lib.fizzy_check_finite.restype = C.c_int
     lib.fizzy_check_finite.argtypes = [vp, C.POINTER(C.c_longlong)]
+    lib.fizzy_count_nonfinite_static.restype = C.c_int
+    lib.fizzy_count_nonfinite_static.argtypes = [C.POINTER(C.c_void_p), C.c_int, C.c_longlong, vp, C.POINTER(C.c_longlong),
+                                                 C.c_char_p, C.c_size_t]
     lib.fizzy_gamma.restype = C.c_double
     lib.fizzy_gamma.argtypes = [vp]
     lib.fizzy_launch_count.restype = C.c_longlong
@@ -142,6 +146,28 @@ def _addr(a):
 def fizzy_workspace_bytes(cfg: dict) -> int:
     g, bc, pr, _keep = structs_from_cfg(cfg)
     return int(_lib.fizzy_workspace_bytes(C.byref(g), C.byref(bc), C.byref(pr)))
+
+
+FIZZY_STATIC_MAX_VALUES = 1 << 27
+FIZZY_STATIC_MAX_FIELDS = 8
+
+
+def fizzy_count_nonfinite_static(fields, n=None, stream=None) -> int:
+    """Number of Inf / NaN values in up to 8 device fields, with no context and no allocation on the library's side
+    (the scratch is an array built into libfizzy.so; see include/fizzy.h for who needs that and for the size limit).
+    `fields`: CUDA tensors of float64 (or raw device addresses, then `n` = values per field is required).  Marshalling
+    only: the addresses go into a ctypes array, the library does the rest.  Run with the fields' device current."""
+    ptrs = [_addr(a) for a in fields]
+    if n is None:
+        n = fields[0].numel() if fields else 0
+        assert all(a.numel() == n for a in fields), "fields of different sizes: pass n"
+    arr = (C.c_void_p * max(len(ptrs), 1))(*ptrs)
+    cnt, err = C.c_longlong(-1), C.create_string_buffer(512)
+    st = _lib.fizzy_count_nonfinite_static(arr, len(ptrs), int(n), stream.cuda_stream if stream is not None else None,
+                                           C.byref(cnt), err, len(err))
+    if st != FIZZY_OK:
+        raise FizzyError(st, err.value.decode())
+    return cnt.value
 
 
 class Fizzy:

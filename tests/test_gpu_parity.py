@@ -37,11 +37,17 @@ CASES = {
 
 
 
-# nx = 1024 on a 1024 x 16 x 8 grid of the 2 pi box has dx/dz = 1/128 (Poisson condition number ~ 128^2 times
-# that of a cubic cell) and max|w| = 1.4e-3 max|u|.  Stage 0 meets the stated 1e-10 on every field; at stages 1
-# and 2 the round-off of the two evaluations, amplified by that conditioning, reaches 1.0e-9 in p and 4.2e-8 in w
-# (measured on the B200; 6e-11 of max|u|), so this one case is held to 1e-7 there.  The same 1024-point
-# transform meets 1e-10 per field at all three stages on cfg4_nx1024_64x64.
+# cfg1_nx1024 (1024 x 16 x 8 cells of the 2 pi box: dy = 64 dx, dz = 128 dx, drop radius 65 dx) is held to 1e-7 instead
+# of 1e-10 at stages 1 and 2 (measured on the B200: 1.0e-9 in p, 4.2e-8 in w = 6e-11 of max|u|; stage 0 meets 1e-10 on
+# every field).  The reason is the case, not a kernel: the ORACLE's own answer moves by 6.6e-9 in w and 1.4e-9 in p when
+# phi changes by <= 1e-20 in the 199 cells with 0 < phi < 1e-13 (psi = eps ln(phi + delta) has condition number
+# eps/(phi + delta); those cells neighbour interface cells across the coarse y and z spacings) --
+# tests/test_oracle_step.py::test_the_1024x16x8_case_cannot_be_defined_to_1e_10 asserts it on the CPU.  Round 3 re-ran
+# the case with two Newton steps in fz_rcp / fz_rsqrt and with an IEEE division for the tridiagonal pivots: the
+# differences to the oracle are the same to every printed digit, so the one-step reciprocals of commit 0699ccd are not the
+# cause.  The same 1024-point transform meets 1e-10 per field at all three stages where y and z are resolved
+# (cfg4_nx1024_64x64), and a oracle built with FMA contraction agrees with the plain one to 8e-13 on this case: the
+# sensitivity is to phi in the far tail only.
 DEGENERATE = {"cfg1_nx1024": 1e-7}
 
 
@@ -106,8 +112,9 @@ def test_full_step_without_reads_in_between(fz, oracle_mod, name):
     for stage in range(3):
         g2.fizzy_rk3_substep(stage, dt)
         f2 = g2.get_fields_numpy()
+    tol2 = 1e-12 if name not in DEGENERATE else tol
     for k in fo:
-        assert field_error(f2[k], fg[k]) <= 1e-12 if name not in DEGENERATE else tol, (name, k, field_error(f2[k], fg[k]))
+        assert field_error(f2[k], fg[k]) <= tol2, (name, k, field_error(f2[k], fg[k]))
     g.close()
     g2.close()
 
@@ -363,3 +370,43 @@ def test_check_finite(fz):
     g.set_fields_numpy(**bad)
     assert g.fizzy_check_finite() == 2
     g.close()
+
+
+@pytest.mark.parametrize("grid", [(8, 8, 12), (64, 32, 12), (64, 32, 67)])
+def test_p_hat_extrapolation_follows_the_hydrostatic_recurrence(fz, grid):
+    """N7 pinned on the CUDA path by a closed form, not by the oracle (the oracle has the same pin in
+    tests/test_oracle_step.py, where the derivation is): a stratified fluid at rest between walls obeys, at every interior
+    w face,  g_new = rho0 G + (1 - rho0/rho_f)(2 g - g_prev),  g = d p/dz,  g = g_prev = 0 at the start -- only with
+    p_hat = 2 p - p_prev, p_prev := p at fizzy_set_fields, and the rotation in the documented order.  Read after every
+    substep (k_correct<false> forms p_hat) and, on a second context, once per RK3 step (k_corr_phi / k_correct<true> do)."""
+    nx, ny, nz = grid
+    cfg = W._base(nx, ny, nz, 1.0, 1.0, 2.0)
+    cfg.update(z_wall=1, rho1=4.0, rho2=1.0, mu1=0.3, mu2=0.1, gz=-1.5, rho_ref=0.0, eps=0.1)
+    zf = 1.0 + np.tanh(1.6 * (np.arange(nz + 1) / nz - 0.5)) / np.tanh(0.8)
+    zf[0], zf[-1] = 0.0, 2.0
+    cfg["zf"] = zf
+    zc = W.cell_centres(cfg)[2]
+    phi = 0.5 * (1.0 - np.tanh((zc - 0.9) / (2.0 * cfg["eps"])))
+    z = np.zeros((nz, ny, nx))
+    f = dict(u=z.copy(), v=z.copy(), w=z.copy(), p=z.copy(), phi=np.ascontiguousarray(phi[:, None, None] + z))
+    rho = cfg["rho2"] + (cfg["rho1"] - cfg["rho2"]) * np.clip(phi, 0.0, 1.0)
+    rho_f = 0.5 * (rho[1:] + rho[:-1])
+    rho0, G = 1.0, cfg["gz"]
+    r = 1.0 - rho0 / rho_f
+    scale = abs(rho_f.max() * G)
+    a, b = fz.Fizzy(cfg), fz.Fizzy(cfg)
+    a.set_fields_numpy(**f)
+    b.set_fields_numpy(**f)
+    g, g_prev = np.zeros_like(rho_f), np.zeros_like(rho_f)
+    dt = 3e-3
+    for sub in range(9):
+        a.fizzy_rk3_substep(sub % 3, dt)
+        b.fizzy_rk3_substep(sub % 3, dt)
+        g, g_prev = rho0 * G + r * (2.0 * g - g_prev), g
+        outs = [a.get_fields_numpy()] + ([b.get_fields_numpy()] if sub % 3 == 2 else [])
+        for out in outs:
+            grad = np.diff(out["p"], axis=0) / np.diff(zc)[:, None, None]
+            assert np.abs(grad - g[:, None, None]).max() <= 1e-11 * scale, (sub, np.abs(grad - g[:, None, None]).max())
+            assert max(np.abs(out[k]).max() for k in "uvw") <= 1e-13
+    a.close()
+    b.close()

@@ -138,3 +138,97 @@ def test_rk3_temporal_order(oracle_mod):
     for k in ("u", "v", "phi"):
         e1, e2 = np.abs(a[k] - b[k]).max(), np.abs(b[k] - c[k]).max()
         assert math.log2(e1 / e2) > 2.7, (k, e1, e2, math.log2(e1 / e2))
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# N7: p_hat = 2 p - p_prev, p_prev := p at fizzy_set_fields, the pressures rotate
+# after every substep.  Pin: a closed-form recurrence that only this reading satisfies.
+#
+# A stratified fluid at rest between walls, phi = phi(z), gravity along z, Gamma = 0, sigma = 0: every right-hand side
+# except gravity vanishes, so u* = a dt G on the w faces (G = gz, rho_ref = 0) and the flow stays at rest (one-dimensional,
+# divergence-free, zero at the walls => w == 0).  Integrating S4 from the bottom wall and inserting into S5 gives, at every
+# interior w face with rho_f = (rho_k + rho_k+1)/2 and g = d p / dz there,
+#       g_new = rho0 G + (1 - rho0/rho_f) g_hat,       g_hat = 2 g - g_prev,      g = g_prev = 0 before the first substep,
+# independent of a and dt.  The fixed point is the hydrostatic gradient rho_f G; where rho_f > rho0 the iteration
+# oscillates towards it with |lambda| = sqrt(1 - rho0/rho_f).  A p_hat = p reading obeys g_new = rho0 G + r g instead, a
+# swapped rotation 2 g_prev - g; both fail below from the second substep on.
+def _hydrostatic_case(stretched):
+    nx, ny, nz = 8, 8, 12
+    cfg = W._base(nx, ny, nz, 1.0, 1.0, 2.0)
+    cfg.update(z_wall=1, rho1=4.0, rho2=1.0, mu1=0.3, mu2=0.1, gz=-1.5, rho_ref=0.0, eps=0.1)
+    if stretched:
+        zf = 1.0 + np.tanh(1.6 * (np.arange(nz + 1) / nz - 0.5)) / math.tanh(0.8)
+        zf[0], zf[-1] = 0.0, 2.0
+        cfg["zf"] = zf
+    zc = W.cell_centres(cfg)[2]
+    phi = 0.5 * (1.0 - np.tanh((zc - 0.9) / (2.0 * cfg["eps"])))          # heavy fluid (phi = 1) below
+    z = np.zeros((nz, ny, nx))
+    f = dict(u=z.copy(), v=z.copy(), w=z.copy(), p=z.copy(), phi=np.ascontiguousarray(phi[:, None, None] + z))
+    return cfg, f, zc
+
+
+@pytest.mark.parametrize("stretched", [False, True])
+def test_p_hat_extrapolation_follows_the_hydrostatic_recurrence(oracle_mod, stretched):
+    cfg, f, zc = _hydrostatic_case(stretched)
+    o = oracle_mod.Oracle(cfg)
+    o.set_fields(**f)
+    rho = cfg["rho2"] + (cfg["rho1"] - cfg["rho2"]) * np.clip(f["phi"][:, 0, 0], 0.0, 1.0)
+    rho_f = 0.5 * (rho[1:] + rho[:-1])
+    rho0, G = min(cfg["rho1"], cfg["rho2"]), cfg["gz"]
+    r = 1.0 - rho0 / rho_f
+    assert r.max() > 0.7 and r.min() < 0.01           # both phases present: lambda from 0 to sqrt(3)/2
+    g, g_prev = np.zeros_like(rho_f), np.zeros_like(rho_f)
+    p_hist = [f["p"], f["p"]]                          # p, p_prev as loaded (p_prev := p)
+    dt = 3e-3
+    for sub in range(9):                               # three full RK3 steps
+        o.substep(sub % 3, dt)
+        out = o.get_fields()
+        g, g_prev = rho0 * G + r * (2.0 * g - g_prev), g
+        grad = np.diff(out["p"], axis=0) / np.diff(zc)[:, None, None]
+        assert np.abs(grad - g[:, None, None]).max() <= 1e-12 * abs(rho_f.max() * G), (sub, np.abs(grad - g[:, None, None]).max())
+        # the flow stays at rest, the pressure is one-dimensional with zero dzf-weighted mean (N17)
+        assert max(np.abs(out[k]).max() for k in "uvw") <= 1e-14
+        assert np.abs(out["p"] - out["p"][:, :1, :1]).max() <= 1e-13
+        # bookkeeping seen through the interface: p_prev is the pressure of the substep before, and the p_hat this
+        # substep used is 2 p - p_prev of the two read-backs before it
+        assert np.array_equal(out["p_prev"], p_hist[0])
+        assert np.abs(o.intermediate("p_hat") - (2.0 * p_hist[0] - p_hist[1])).max() <= 1e-14 * max(1.0, np.abs(p_hist[0]).max())
+        p_hist = [out["p"], p_hist[0]]
+    # after nine substeps the gradient is near the hydrostatic one but not there yet (|lambda|^9 ~ 0.27 in the heavy fluid):
+    # the recurrence, not the fixed point, is what was compared
+    assert 0.01 < np.abs(g - rho_f * G).max() / abs(rho_f.max() * G) < 0.5
+    o.close()
+
+
+def test_the_1024x16x8_case_cannot_be_defined_to_1e_10(oracle_mod):
+    """Why tests/test_gpu_parity.py holds its `cfg1_nx1024` case (1024 x 16 x 8 cells of the 2 pi box, dy = 64 dx,
+    dz = 128 dx, drop radius 65 dx) to 1e-7 instead of BASELINE.json's 1e-10 at stages 1 and 2: the ORACLE's own result is
+    not defined to 1e-10 there.  psi = eps ln((phi + delta)/(1 - phi + delta)) (N2, delta = 1e-100) has the condition
+    number eps/(phi + delta) with respect to phi, and this drop is wide enough (R = 65 eps) for phi to fall to 1e-13 ...
+    1e-17 within the grid; such cells sit next to interface cells across the coarse y and z spacings, so their psi enters
+    n_hat and kappa of cells where grad phi is O(1).  Changing phi by at most 1e-20 -- one ten-thousandth of an ulp of
+    1.0, far below anything the N19 norm of phi can see -- in those cells moves w by > 1e-9 and p by > 1e-10 (measured:
+    6.6e-9 and 1.4e-9; 1e-18 gives 6.7e-7 and 1.4e-7).  The library differs from the oracle by 4.2e-8 in w and 1.0e-9 in
+    p on this case, bit-identically with two Newton steps or an IEEE division in its reciprocals (round 3, DESIGN.md
+    section 3), and by <= 1e-10 on the same 1024-point transform with resolved y and z (cfg4_nx1024_64x64)."""
+    cfg, f, dt, _ = W.make(1, grid=(1024, 16, 8), ndrops=1)
+    phi = f["phi"]
+    tiny = (phi > 0.0) & (phi < 1e-13)
+    assert 100 < tiny.sum() < 1000 and phi.max() < 0.9995          # a thin shell of cells; no saturation on the phi = 1 side
+    rng = np.random.default_rng(5)
+    phi2 = phi.copy()
+    phi2[tiny] = np.maximum(phi2[tiny] + 1e-20 * rng.uniform(-1.0, 1.0, int(tiny.sum())), 0.0)
+    assert np.abs(phi2 - phi).max() <= 1e-20
+    a, b = oracle_mod.Oracle(cfg), oracle_mod.Oracle(cfg)
+    a.set_fields(**f)
+    b.set_fields(**dict(f, phi=phi2))
+    worst = {"w": 0.0, "p": 0.0}
+    for s in range(3):
+        a.substep(s, dt)
+        b.substep(s, dt)
+        fa, fb = a.get_fields(), b.get_fields()
+        for k in worst:
+            worst[k] = max(worst[k], np.abs(fb[k] - fa[k]).max() / np.abs(fa[k]).max())
+    a.close(); b.close()
+    assert worst["w"] > 1e-9 and worst["p"] > 1e-10, worst
+    assert worst["w"] < 1e-7, worst                                  # ... and the GPU test's 1e-7 is not a blank cheque

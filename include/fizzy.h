@@ -45,7 +45,8 @@ typedef enum {
     FIZZY_EINVAL = 1, /* bad argument (see each call) */
     FIZZY_ENOMEM = 2, /* workspace too small / host allocation failed */
     FIZZY_ECUDA = 3,  /* CUDA runtime error; text via fizzy_last_error */
-    FIZZY_ESTATE = 4  /* call out of order (substep before set_fields, stage sequence) */
+    FIZZY_ESTATE = 4, /* call out of order (substep before set_fields, stage sequence) */
+    FIZZY_ENOCONV = 5 /* pressure solver 1 only: the iterative solve missed rtol within max_iter (no CUDA call failed) */
 } fizzy_status;
 
 /* Grid ("3D Cartesian grid").  nx, ny powers of two in [8, 1024]; nz >= 4;
@@ -198,7 +199,11 @@ size_t fizzy_varcoef_workspace_bytes(const fizzy_ctx *ctx);
  *             (to rtol, at most max_iter iterations), then  u = u* - a dt (1/rho_f) d p_new;  no extrapolated pressure, no
  *             reference density.  dev_work: caller-owned DEVICE scratch of fizzy_varcoef_workspace_bytes(ctx) bytes, 256-byte
  *             aligned, which must stay valid while solver 1 is selected.  Every substep then synchronises the stream, CUDA
- *             graph replay is bypassed, and a solve that misses rtol within max_iter makes the substep return FIZZY_ECUDA.
+ *             graph replay is bypassed, and a solve that misses rtol within max_iter makes the substep return FIZZY_ENOCONV.  At
+ *             that point phi, T, the RK histories and u** are already those of the new substep but the velocity is not yet
+ *             corrected and the stage counter has not moved: the context cannot be retried as it is -- reload it with
+ *             fizzy_set_fields (then e.g. raise max_iter).
+ *   Going back from solver 1 to solver 0 re-forms p_hat = 2 p - p_prev (N7) from the pressures of the last two substeps.
  * Only between RK3 steps (FIZZY_ESTATE otherwise).  FIZZY_EINVAL / FIZZY_ENOMEM as for fizzy_poisson_solve_varcoef. */
 fizzy_status fizzy_set_pressure_solver(fizzy_ctx *ctx, int solver, void *dev_work, size_t work_bytes, double rtol,
                                        int max_iter);

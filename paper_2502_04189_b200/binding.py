@@ -13,8 +13,8 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libfizzy.so")
 
-FIZZY_OK, FIZZY_EINVAL, FIZZY_ENOMEM, FIZZY_ECUDA, FIZZY_ESTATE = range(5)
-_STATUS = {0: "FIZZY_OK", 1: "FIZZY_EINVAL", 2: "FIZZY_ENOMEM", 3: "FIZZY_ECUDA", 4: "FIZZY_ESTATE"}
+FIZZY_OK, FIZZY_EINVAL, FIZZY_ENOMEM, FIZZY_ECUDA, FIZZY_ESTATE, FIZZY_ENOCONV = range(6)
+_STATUS = {0: "FIZZY_OK", 1: "FIZZY_EINVAL", 2: "FIZZY_ENOMEM", 3: "FIZZY_ECUDA", 4: "FIZZY_ESTATE", 5: "FIZZY_ENOCONV"}
 
 EXPORTS = ["fizzy_workspace_bytes", "fizzy_create", "fizzy_destroy", "fizzy_set_fields",
            "fizzy_rk3_substep", "fizzy_poisson_solve", "fizzy_get_fields", "fizzy_gamma", "fizzy_diagnostics",

@@ -11,7 +11,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "libfizzy.so")
 SOURCES = ["fizzy_api.cu", "fizzy_static.cu"]
-HEADERS = ["fz_common.cuh", "fz_stencil.cuh", "fz_momentum.cuh", "fz_fft.cuh", "fz_fftx.cuh", "fz_spectral.cuh", "fz_linefft.cuh", "fz_iface.cuh", "fz_diag.cuh"]
+HEADERS = ["fz_common.cuh", "fz_stencil.cuh", "fz_momentum.cuh", "fz_fft.cuh", "fz_fftx.cuh", "fz_spectral.cuh", "fz_linefft.cuh", "fz_iface.cuh", "fz_diag.cuh", "fz_mg.cuh"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-std=c++17", "-O3", "-lineinfo",
               "-shared", "-Xcompiler", "-fPIC", "-cudart", "static"]
 

@@ -181,7 +181,7 @@ cudaEvent_t take_event(fizzy_ctx *c)
 {
     if (!c->pool.empty()) { cudaEvent_t e = c->pool.back(); c->pool.pop_back(); return e; }
     cudaEvent_t e = nullptr;
-    cudaEventCreate(&e);
+    if (cudaEventCreate(&e) != cudaSuccess) { cudaGetLastError(); e = nullptr; }   // no event: this launch goes untimed
     return e;
 }
 
@@ -191,7 +191,7 @@ cudaEvent_t take_event(fizzy_ctx *c)
     do {                                                                \
         if (c->timing) {                                                \
             FzTimed t_; t_.id = (id_); t_.e0 = take_event(c); t_.e1 = take_event(c); \
-            cudaEventRecord(t_.e0, c->stream);                          \
+            if (t_.e0) cudaEventRecord(t_.e0, c->stream);               \
             c->pending.push_back(t_);                                   \
         }                                                               \
     } while (0)
@@ -199,7 +199,7 @@ cudaEvent_t take_event(fizzy_ctx *c)
 #define FZ_LAUNCHED(id_)                                                \
     do {                                                                \
         ++c->launches;                                                  \
-        if (c->timing) cudaEventRecord(c->pending.back().e1, c->stream); \
+        if (c->timing && c->pending.back().e1) cudaEventRecord(c->pending.back().e1, c->stream); \
         cudaError_t e_ = cudaPeekAtLastError();                         \
         if (e_ != cudaSuccess) return cuda_fail(c, e_, FZK_NAME[id_]);  \
     } while (0)
@@ -382,7 +382,7 @@ extern "C" fizzy_status fizzy_destroy(fizzy_ctx *c)
 {
     if (!c) return FIZZY_EINVAL;
     cudaStreamSynchronize(c->stream);
-    for (FzTimed &t : c->pending) { cudaEventDestroy(t.e0); cudaEventDestroy(t.e1); }
+    for (FzTimed &t : c->pending) { if (t.e0) cudaEventDestroy(t.e0); if (t.e1) cudaEventDestroy(t.e1); }
     for (cudaEvent_t e : c->pool) cudaEventDestroy(e);
     for (cudaGraphExec_t g : c->gexec)
         if (g) cudaGraphExecDestroy(g);
@@ -405,9 +405,9 @@ extern "C" fizzy_status fizzy_timing_get(fizzy_ctx *c, int index, const char **n
         FZ_CUDA(cudaStreamSynchronize(c->stream));
         for (FzTimed &t : c->pending) {
             float ms = 0.f;
-            if (cudaEventElapsedTime(&ms, t.e0, t.e1) == cudaSuccess) { c->t_ms[t.id] += ms; ++c->t_n[t.id]; }
-            c->pool.push_back(t.e0);
-            c->pool.push_back(t.e1);
+            if (t.e0 && t.e1 && cudaEventElapsedTime(&ms, t.e0, t.e1) == cudaSuccess) { c->t_ms[t.id] += ms; ++c->t_n[t.id]; }
+            if (t.e0) c->pool.push_back(t.e0);
+            if (t.e1) c->pool.push_back(t.e1);
         }
         c->pending.clear();
     }
@@ -685,7 +685,10 @@ extern "C" fizzy_status fizzy_rk3_substep(fizzy_ctx *c, int stage, double dt)
         double relres = 0.0;
         s = fizzy_poisson_solve_varcoef(c, c->pn, nullptr, c->pn, c->mg_work, c->mg_bytes, c->mg_rtol, c->mg_maxit, &iters, &relres);
         if (s != FIZZY_OK) return s;
-        if (!(relres <= c->mg_rtol)) return fail(c, FIZZY_ECUDA, "fizzy_rk3_substep: the variable-coefficient pressure solve did not reach rtol within max_iter");
+        // (the solve stops on rr <= rtol^2 bb; relres is sqrt(rr/bb): one rounding of slack so that the two tests agree)
+        if (!(relres <= c->mg_rtol * (1.0 + 1e-12)))
+            return fail(c, FIZZY_ENOCONV, "fizzy_rk3_substep: the variable-coefficient pressure solve did not reach rtol within max_iter; "
+                                          "the context is part-way through the substep: reload it with fizzy_set_fields");
         FZ_TB(FZK_CORRECT);
         if (stage == 2)
             k_correct_var<true><<<grid, block, 0, c->stream>>>(P, c->us, c->vs, c->ws, c->pn, c->phi, c->u, c->v, c->w, as * dt, c->scal);
@@ -836,6 +839,8 @@ extern "C" fizzy_status fizzy_rk3_step(fizzy_ctx *c, double dt)
         if (c->gexec[par]) { cudaGraphExecDestroy(c->gexec[par]); c->gexec[par] = nullptr; }
         // the capture itself executes nothing: remember the buffer rotation, capture, restore, then replay below
         double *sv[] = {c->phi, c->phin, c->p, c->pp, c->pn, c->T, c->Tn};
+        const bool sv_pending = c->corr_pending;   // false here (a full step ends with k_correct<true>), and false again
+        const double sv_coef = c->corr_coef;       // after three captured substeps; restored for a capture that fails midway
         const long long l0 = c->launches;
         cudaGraph_t g = nullptr;
         FZ_CUDA(cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeThreadLocal));
@@ -845,6 +850,8 @@ extern "C" fizzy_status fizzy_rk3_step(fizzy_ctx *c, double dt)
         c->launches = l0;
         c->phi = sv[0]; c->phin = sv[1]; c->p = sv[2]; c->pp = sv[3]; c->pn = sv[4]; c->T = sv[5]; c->Tn = sv[6];
         c->next_stage = 0;
+        c->corr_pending = sv_pending;
+        c->corr_coef = sv_coef;
         if (s != FIZZY_OK) { if (g) cudaGraphDestroy(g); return s; }
         if (ce != cudaSuccess) return cuda_fail(c, ce, "cudaStreamEndCapture");
         const cudaError_t ie = cudaGraphInstantiate(&c->gexec[par], g, 0);
@@ -914,6 +921,15 @@ extern "C" fizzy_status fizzy_set_pressure_solver(fizzy_ctx *c, int solver, void
             return fail(c, FIZZY_EINVAL, "solver 1 needs 256-byte aligned dev_work, rtol > 0, max_iter >= 1");
         if (work_bytes < mg_plan(c).doubles * sizeof(double)) return fail(c, FIZZY_ENOMEM, "dev_work is smaller than fizzy_varcoef_workspace_bytes");
         c->mg_work = dev_work; c->mg_bytes = work_bytes; c->mg_rtol = rtol; c->mg_maxit = max_iter;
+    }
+    if (c->solver == 1 && solver == 0 && c->varrho && c->fields_set) {
+        // the solver-1 substeps rotate p and p_prev but never write p_hat; the splitting's predictor reads it from
+        // c->phat (N7), so form 2 p - p_prev of the current pressures before the first splitting substep
+        dim3 grid, block;
+        cell_launch(c, grid, block);
+        FZ_TB(FZK_OTHER);
+        k_phat<<<grid, block, 0, c->stream>>>(c->P, c->p, c->pp, c->phat);
+        FZ_LAUNCHED(FZK_OTHER);
     }
     c->solver = solver;
     return FIZZY_OK;

@@ -189,6 +189,19 @@ def stable_dt(cfg, u, v, w) -> float:
     return 0.5 * min(lims)
 
 
+# Host memory a CPU comparison run of configs[4] at its own 1024x512x512 needs (about 40 ghost-padded fp64 arrays of
+# 2.19 GB, a complex work array, the inputs and two sets of outputs).  Below it the full-size parity test falls back to
+# 1024x512x256; `cfg5_parity_grid` is the one place that decides, so that the test and smoke() report the same branch.
+CFG5_FULL_HOST_GB = 150.0
+
+
+def cfg5_parity_grid(available_gb: float):
+    """(grid, ndrops, label) of the configs[4] full-size parity case on a host with `available_gb` of free memory."""
+    if available_gb >= CFG5_FULL_HOST_GB:
+        return None, None, "1024x512x512"
+    return (1024, 512, 256), 32, "1024x512x256"
+
+
 def make(index: int, grid=None, ndrops=None, radius=None):
     """Build configuration `index` (0..4).  `grid=(nx,ny,nz)`, `ndrops`, `radius` override the
     BASELINE.json sizes for small parity cases (same recipe, same parameters).

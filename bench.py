@@ -10,8 +10,9 @@ target is quoted on), synthetic seeded inputs from paper_2502_04189_b200.workloa
 N>1: replicas only: every rank runs the same workload on its own GPU,
 no data-path collective; value = cells*substeps of all ranks / max-over-ranks time.
 
-One JSON line on stdout (rank 0).  `--impl reference` times the CPU oracle on a bounded sample
-(the same recipe at --cpu-grid^3, the grid the `cpu_baseline` leg of the default arm uses too).
+One JSON line on stdout (rank 0).  `--impl reference` times the CPU oracle, as it stands, on the SAME workload
+(config 4 at 512^3: about 20 s per RK3 step on 16 cores); `cpu_baseline` of the default arm is one such step.  A smaller
+sample only with an explicit --cpu-grid N (or when the host has too little memory), and then config.workload says so.
 
 Timed regions: (1) `value`: K steps, inputs resident in HBM, per-kernel timing OFF, CUDA events on the
 library's stream; (2) a second, shorter pass with fizzy_timing_enable for the per-kernel table and the
@@ -35,7 +36,7 @@ sys.path.insert(0, ROOT)
 
 from paper_2502_04189_b200 import workloads as W  # noqa: E402
 
-TRAFFIC_CSV, TRAFFIC_MD = "r2e_traffic.csv", "r2e_ncu_full.md"
+TRAFFIC_CSV, TRAFFIC_MD = "r3_traffic.csv", "r3_ncu_full.md"
 METRIC = "fp64 Mcell-substeps/s per RK3 step"
 UNIT = "Mcell-substeps/s"
 
@@ -64,6 +65,18 @@ def algorithmic_bytes_per_cell(cfg):
     if heat:
         b["k_temp_update"] = 64.0
     return b
+
+
+def moved_bytes_per_cell(cfg):
+    """Bytes a launch really moves, per stage (0, 1, 2), where they differ from the undiscounted model above: stage 0
+    reads no RK history (zeta = 0) and stage 2 writes none (the next stage 0 does not read it).  None = no launch."""
+    a = algorithmic_bytes_per_cell(cfg)
+    m = a["k_momentum"]
+    c = a["k_corr_phi"]
+    return {"k_momentum": [m - 24.0, m, m - 24.0],          # h x3 not read / not written
+            "k_phi_update": [a["k_phi_update"] - 8.0, None, None],   # stage 0 only: h_phi not read
+            "k_corr_phi": [None, c, c - 8.0],                # stage 2 writes no h_phi
+            "k_correct": [None, None, a["k_correct"]]}
 
 
 def substep_model_bytes(cfg):
@@ -139,29 +152,55 @@ class ClockSampler(threading.Thread):
                 "samples": len(sm)}
 
 
+ORACLE_GB_PER_MCELL = 0.45   # host memory of the oracle: ~40 ghost-padded arrays + FFT work + inputs/outputs, per 1e6 cells
+
+
+def oracle_sample_fits(cells):
+    import psutil
+    return psutil.virtual_memory().available / 1e9 >= ORACLE_GB_PER_MCELL * cells / 1e6
+
+
+def oracle_sample(args):
+    """(cfg, fields, dt, workload label, same_config) of the oracle runs: the bench's own workload unless --cpu-grid N asks
+    for the same recipe at N^3 or the host cannot hold the oracle's arrays (then 256^3, and the label says so)."""
+    grid = tuple(args.grid) if args.grid else W.DEFAULT_GRIDS[args.workload]
+    cells = grid[0] * grid[1] * grid[2]
+    n = args.cpu_grid
+    if n == 0 and not oracle_sample_fits(cells):
+        n = 256
+    if n == 0:
+        cfg, f, dt, _ = W.make(args.workload, grid=tuple(args.grid) if args.grid else None)
+        return cfg, f, dt, cfg["name"], True
+    cfg, f, dt, _ = W.make(args.workload, grid=(n, n, n), ndrops=max(1, 200 // max(1, 512 // n) ** 3))
+    return cfg, f, dt, "%s recipe at %d^3 (NOT the bench grid)" % (W.NAMES[args.workload], n), False
+
+
 def run_reference(args, rank):
-    """The CPU oracle as it stands, on the host cores, on a bounded sample of the workload."""
+    """The CPU oracle as it stands, on the host cores, on the bench's own workload; a step is one RK3 step.  At 512^3 a
+    step takes about 20 s, so the warm-up is capped at one step (a CPU program has nothing to warm beyond its first touch of
+    memory); the line reports the warm-up that ran."""
     if rank != 0:
         return
     import oracle
     oracle.build()
-    n = args.cpu_grid
-    cfg, f, dt, _ = W.make(args.workload, grid=(n, n, n), ndrops=max(1, 200 // (512 // n) ** 3))
+    cfg, f, dt, label, same = oracle_sample(args)
     o = oracle.Oracle(cfg)
     o.set_fields(**f)
-    for _ in range(args.warmup):
+    warm = min(args.warmup, 1)
+    for _ in range(warm):
         o.step(dt)
     t0 = time.perf_counter()
     for _ in range(args.steps):
         o.step(dt)
     el = time.perf_counter() - t0
-    cells = n ** 3
+    cells = cfg["nx"] * cfg["ny"] * cfg["nz"]
     value = cells * 3 * args.steps / el / 1e6
-    sample = "config %d recipe at %d^3, %d RK3 steps" % (args.workload, n, args.steps)
+    sample = "%s, %d x %d x %d cells, %d RK3 steps in %.1f s" % (label, cfg["nx"], cfg["ny"], cfg["nz"], args.steps, el)
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
-            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * el / args.steps,
+            "steps": args.steps, "warmup": warm, "ms_per_step": 1e3 * el / args.steps,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": W.NAMES[args.workload], "sample": sample},
+            "config": {"workload": label, "grid": [cfg["nx"], cfg["ny"], cfg["nz"]], "same_config_as_default_arm": same,
+                       "sample": sample},
             "cpu_baseline": {"value": value, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
                              "cpu_model": cpu_model(), "sample": sample},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
@@ -169,20 +208,66 @@ def run_reference(args, rank):
     print(json.dumps(line), flush=True)
 
 
-def cpu_baseline(args):
-    """Oracle timed on a bounded sample (one RK3 step of the same recipe at --cpu-grid^3)."""
+def cpu_baseline(args, sample=None):
+    """Oracle timed on ONE RK3 step of the bench's own workload (see oracle_sample)."""
     import oracle
     oracle.build()
-    n = args.cpu_grid
-    cfg, f, dt, _ = W.make(args.workload, grid=(n, n, n), ndrops=max(1, 200 // (512 // n) ** 3))
+    cfg, f, dt, label, same = sample if sample is not None else oracle_sample(args)
     o = oracle.Oracle(cfg)
     o.set_fields(**f)
     t0 = time.perf_counter()
     o.step(dt)
     el = time.perf_counter() - t0
     o.close()
-    return {"value": n ** 3 * 3 / el / 1e6, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
-            "cpu_model": cpu_model(), "sample": "config %d recipe at %d^3, 1 RK3 step, %.1f s" % (args.workload, n, el)}
+    cells = cfg["nx"] * cfg["ny"] * cfg["nz"]
+    return {"value": cells * 3 / el / 1e6, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
+            "cpu_model": cpu_model(), "same_config": same,
+            "sample": "%s, %d x %d x %d cells, 1 RK3 step, %.1f s" % (label, cfg["nx"], cfg["ny"], cfg["nz"], el)}
+
+
+def other_config(torch, Fizzy, index, device, peak, steps=5, warmup=3):
+    """Device-resident throughput of another BASELINE.json config at its own size (the variable-density / wall / heat
+    variants of the kernels, which the headline workload does not exercise): same timing rules as `value`."""
+    t0 = time.perf_counter()
+    cfg, f, dt, _ = W.make(index)
+    gen_s = time.perf_counter() - t0
+    cells = cfg["nx"] * cfg["ny"] * cfg["nz"]
+    fz = Fizzy(cfg, device=device)
+    names = ["u", "v", "w", "p", "phi"] + (["T"] if cfg["heat"] else [])
+    for k in names:      # one field at a time: at 1024x512x512 the workspace leaves little room for staging copies
+        t = torch.from_numpy(f[k]).to(device)
+        fz.fizzy_set_fields(**{k: t})
+        torch.cuda.synchronize()
+        del t
+    del f
+    for _ in range(warmup):
+        fz.step(dt)
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(fz.stream)
+    for _ in range(steps):
+        fz.step(dt)
+    e1.record(fz.stream)
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1)
+    finite = fz.fizzy_check_finite() == 0
+    fz.fizzy_timing_enable(True)
+    fz.fizzy_timing_get(reset=True)
+    fz.step(dt)
+    per_kernel = fz.fizzy_timing_get(reset=True)
+    fz.close()
+    bpc = algorithmic_bytes_per_cell(cfg)
+    sub_ms = ms / (3 * steps)
+    gbs = substep_model_bytes(cfg) * cells / (sub_ms * 1e-3) / 1e9
+    kern = {}
+    for name, (tot, n) in per_kernel.items():
+        if name in bpc and n:
+            g = bpc[name] * cells / (tot / n * 1e-3) / 1e9
+            kern[name] = {"ms_per_launch": round(tot / n, 4), "algorithmic_B_per_cell": round(bpc[name], 2), "frac": round(g / peak, 4)}
+    return {"workload": cfg["name"], "grid": [cfg["nx"], cfg["ny"], cfg["nz"]], "steps": steps, "warmup": warmup,
+            "value": cells * 3 * steps / (ms * 1e-3) / 1e6, "unit": UNIT, "ms_per_substep": round(sub_ms, 4),
+            "model_B_per_cell": substep_model_bytes(cfg), "achieved_GBs": round(gbs, 1), "frac": round(gbs / peak, 4),
+            "finite": finite, "generation_s": round(gen_s, 1), "kernels": kern}
 
 
 def cufft_compare(torch, cfg, per_kernel, device):
@@ -296,7 +381,10 @@ def main():
     ap.add_argument("--workload", type=int, default=3, help="BASELINE.json config index (0-based)")
     ap.add_argument("--grid", type=int, nargs=3, default=None, help="override nx ny nz (debug)")
     ap.add_argument("--impl", default="fizzy", choices=["fizzy", "reference"])
-    ap.add_argument("--cpu-grid", type=int, default=256, help="oracle sample grid (cpu_baseline and --impl reference)")
+    ap.add_argument("--cpu-grid", type=int, default=0,
+                    help="0 (default): the oracle runs the bench's own workload; N: the same recipe at N^3 instead (labelled)")
+    ap.add_argument("--other-configs", type=int, nargs="*", default=[2, 4],
+                    help="BASELINE.json config indices timed at their own size after the headline workload (N = 1 only)")
     ap.add_argument("--no-cufft", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
@@ -386,14 +474,22 @@ def main():
     # ---------------- roofline of the dominant kernel + per-kernel table ----------------
     peak, peak_src = measured_peak_gbs()
     bpc = algorithmic_bytes_per_cell(cfg)
+    moved = moved_bytes_per_cell(cfg)
     table = []
     for name, (tot_ms, n) in per_kernel.items():
         if name in bpc and n:
             avg = tot_ms / n
             gbs = bpc[name] * cells / (avg * 1e-3) / 1e9
-            table.append({"kernel": name, "ms_per_launch": round(avg, 4), "launches": n,
-                          "share": tot_ms, "algorithmic_B_per_cell": round(bpc[name], 2),
-                          "achieved_GBs": round(gbs, 1), "frac": round(gbs / peak, 4)})
+            row = {"kernel": name, "ms_per_launch": round(avg, 4), "launches": n,
+                   "share": tot_ms, "algorithmic_B_per_cell": round(bpc[name], 2),
+                   "achieved_GBs": round(gbs, 1), "frac": round(gbs / peak, 4)}
+            if name in moved:   # mean over the stages that launch it: what really crosses HBM
+                per_stage = [b for b in moved[name] if b is not None]
+                mv = sum(per_stage) / len(per_stage)
+                row["bytes_moved_B_per_cell"] = round(mv, 2)
+                row["bytes_moved_per_stage"] = moved[name]
+                row["frac_moved"] = round(mv * cells / (avg * 1e-3) / 1e9 / peak, 4)
+            table.append(row)
     tot = sum(r["share"] for r in table) or 1.0
     for r in table:
         r["share"] = round(r["share"] / tot, 4)
@@ -404,16 +500,24 @@ def main():
     roofline = None
     if top:
         roofline = {"bound": "hbm", "kernel": top["kernel"], "achieved": top["achieved_GBs"], "peak": peak,
-                    "unit": "GB/s", "frac": top["frac"], "traffic": None, "peak_source": peak_src}
+                    "unit": "GB/s", "frac": top["frac"], "traffic": None, "peak_source": peak_src,
+                    "algorithmic_B_per_cell": top["algorithmic_B_per_cell"],
+                    "bytes_moved_B_per_cell": top.get("bytes_moved_B_per_cell", top["algorithmic_B_per_cell"]),
+                    "frac_moved": top.get("frac_moved", top["frac"])}
     # ncu DRAM traffic per launch of the dominant kernel: NOT measured in this run (a number printed under a
     # profiler is never a bench value); it is the committed ncu capture named in `traffic_source`
     try:
         with open(os.path.join(ROOT, "profiles", TRAFFIC_CSV)) as fh:
+            per_stage = {}
             for ln in fh:
                 parts = ln.strip().split(",")
-                if roofline and len(parts) == 3 and parts[0] == cfg["name"] and parts[1] == roofline["kernel"]:
-                    roofline["traffic"] = float(parts[2])
-                    roofline["traffic_source"] = "ncu --set full capture, profiles/%s (see profiles/%s)" % (TRAFFIC_CSV, TRAFFIC_MD)
+                if roofline and len(parts) == 4 and parts[0] == cfg["name"] and parts[1] == roofline["kernel"]:
+                    per_stage[int(parts[2])] = float(parts[3])
+            if per_stage:   # the same average the `frac` is taken over: one launch per stage
+                roofline["traffic"] = sum(per_stage.values()) / len(per_stage)
+                roofline["traffic_per_stage"] = [per_stage.get(q) for q in range(3)]
+                roofline["traffic_source"] = ("mean of the stage-0/1/2 launches of one RK3 step, ncu --set full capture, "
+                                              "profiles/%s (see profiles/%s)" % (TRAFFIC_CSV, TRAFFIC_MD))
     except Exception:
         pass
 
@@ -449,11 +553,26 @@ def main():
         if dist is not None:
             dist.destroy_process_group()
         return
-    cpu = None
+    cpu, others = None, None
+    fz.close()
+    del dev
+    if not args.no_e2e:
+        del hin, hout
+    torch.cuda.empty_cache()
     if world == 1 and not args.no_cpu_baseline:
-        fz.close()
-        del dev
-        cpu = cpu_baseline(args)
+        same = args.cpu_grid == 0
+        cpu = cpu_baseline(args, (cfg, f, dt, cfg["name"], True) if same and oracle_sample_fits(cells) else None)
+    del f
+    if world == 1 and args.other_configs and not args.grid and not args.pressure_solver:
+        others = []
+        for index in args.other_configs:
+            if index == args.workload:
+                continue
+            try:
+                others.append(other_config(torch, Fizzy, index, "cuda:%d" % local_rank, peak))
+            except Exception as exc:   # e.g. not enough device or host memory for config 5 on this box: say so, keep the line
+                others.append({"workload": W.NAMES[index], "unavailable": "%s: %s" % (type(exc).__name__, str(exc)[:200])})
+            torch.cuda.empty_cache()
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
@@ -470,7 +589,7 @@ def main():
             "roofline_substep": {"bound": "hbm", "model_B_per_cell": substep_model_bytes(cfg),
                                  "ms_per_substep": sub_ms, "achieved": round(sub_gbs, 1), "peak": peak,
                                  "unit": "GB/s", "frac": round(sub_gbs / peak, 4)},
-            "kernels": table, "cufft_compare": cufft, "graph_compare": graphs, "cpu_baseline": cpu}
+            "kernels": table, "other_configs": others, "cufft_compare": cufft, "graph_compare": graphs, "cpu_baseline": cpu}
     print(json.dumps(line), flush=True)
     if dist is not None:
         dist.destroy_process_group()

@@ -11,10 +11,12 @@
  * leg may build, load or call this.  It shares no code with the CUDA path.
  *
  * Parity unpinned (any consistent choice passes every check we have; fixed by DESIGN.md):
- *   N6  (which phi feeds S3), N7 (pressure extrapolation p_hat = 2p - p_prev),
+ *   N6  (which phi feeds S3),
  *   N9  (non-conservative form of the mass-consistent regularisation-flux term;
  *        pinned only by: vanishes for rho1 == rho2, exact for linear velocity),
  *   N14 (non-conservative temperature equation).
+ * N7 (pressure extrapolation p_hat = 2p - p_prev and the rotation of p, p_prev) is pinned since round 3 by the
+ * closed-form hydrostatic recurrence of tests/test_oracle_step.py.
  *
  * Layout: all field arrays are nx*ny*nz doubles, x fastest: idx = i + nx*(j + ny*k).
  * u[i,j,k] sits on the x-face between cells i and i+1, v on the y-face between j and

@@ -40,6 +40,15 @@ extern "C" {
 
 typedef struct fizzy_ctx fizzy_ctx; /* opaque, owned by the library */
 
+/* Version of this interface.  It goes up whenever a call changes what it reads or writes through an unchanged signature:
+ *   1  round 1;   2  fizzy_diagnostics writes 8 doubles (was 6: the two Nusselt numbers were added);
+ *   3  FIZZY_ENOCONV, fizzy_count_nonfinite_static.
+ * A caller built against an older header compares FIZZY_ABI_VERSION (its compile-time value) with fizzy_abi_version() (the
+ * loaded library's) before the first call and refuses to run on a mismatch -- e.g. a 6-double buffer handed to a version-2
+ * fizzy_diagnostics would be overrun by 16 bytes. */
+#define FIZZY_ABI_VERSION 3
+int fizzy_abi_version(void);
+
 typedef enum {
     FIZZY_OK = 0,
     FIZZY_EINVAL = 1, /* bad argument (see each call) */
@@ -217,7 +226,8 @@ fizzy_status fizzy_get_fields(fizzy_ctx *ctx, double *u, double *v, double *w, d
                               double *phi, double *T, double *p_prev);
 
 /* Run-time diagnostics of the current state (definitions in DESIGN.md 10), one pass
- * over the fields and a fixed-order (deterministic) reduction.  `out` = 8 HOST doubles, dV = dx*dy*dzf[k]:
+ * over the fields and a fixed-order (deterministic) reduction.  `out` = 8 HOST doubles (6 before FIZZY_ABI_VERSION 2),
+ * dV = dx*dy*dzf[k]:
  *   out[0] = sum phi dV (volume of fluid 1)        out[1] = 1/2 sum rho(phi) |u_c|^2 dV, u_c = cell-centred mean
  *   out[2] = max over faces of max(|u|,|v|,|w|)    out[3] = max |D(u)|
  *   out[4] = sum |grad phi| dV (central differences: area of the diffuse interface)

@@ -21,7 +21,7 @@ EXPORTS = ["fizzy_workspace_bytes", "fizzy_create", "fizzy_destroy", "fizzy_set_
            "fizzy_launch_count", "fizzy_last_error", "fizzy_timing_enable", "fizzy_timing_get",
            "fizzy_rk3_step", "fizzy_graph_enable", "fizzy_stable_dt", "fizzy_check_finite",
            "fizzy_varcoef_workspace_bytes", "fizzy_poisson_solve_varcoef", "fizzy_set_pressure_solver",
-           "fizzy_count_nonfinite_static"]
+           "fizzy_count_nonfinite_static", "fizzy_abi_version"]
 
 
 class FizzyGrid(C.Structure):
@@ -90,6 +90,8 @@ def load_library(path: str = LIB_PATH) -> C.CDLL:
     lib.fizzy_count_nonfinite_static.restype = C.c_int
     lib.fizzy_count_nonfinite_static.argtypes = [C.POINTER(C.c_void_p), C.c_int, C.c_longlong, vp, C.POINTER(C.c_longlong),
                                                  C.c_char_p, C.c_size_t]
+    lib.fizzy_abi_version.restype = C.c_int
+    lib.fizzy_abi_version.argtypes = []
     lib.fizzy_gamma.restype = C.c_double
     lib.fizzy_gamma.argtypes = [vp]
     lib.fizzy_launch_count.restype = C.c_longlong
@@ -105,6 +107,10 @@ def load_library(path: str = LIB_PATH) -> C.CDLL:
 
 
 _lib = load_library()
+FIZZY_ABI_VERSION = 3   # the version this binding was written against (include/fizzy.h)
+if _lib.fizzy_abi_version() != FIZZY_ABI_VERSION:
+    raise ImportError("libfizzy.so has interface version %d, this binding expects %d: rebuild with "
+                      "`python -m paper_2502_04189_b200.build`" % (_lib.fizzy_abi_version(), FIZZY_ABI_VERSION))
 
 
 def structs_from_cfg(cfg: dict):
@@ -211,10 +217,14 @@ class Fizzy:
             raise FizzyError(st, text)
 
     def close(self):
-        if getattr(self, "_h", None):
-            with self._on_device():
-                _lib.fizzy_destroy(self._h)
+        h = getattr(self, "_h", None)
+        if h:
             self._h = None
+            try:
+                with self._on_device():
+                    _lib.fizzy_destroy(h)
+            except Exception:   # called from __del__ at interpreter shutdown with torch already torn down: the process is ending
+                pass
 
     __del__ = close
 

@@ -39,10 +39,10 @@ struct Carver {  // hands out 256-byte aligned pieces of the workspace (or just 
 }  // namespace
 
 enum FzKernelId { FZK_LATCH, FZK_PHI, FZK_CORRPHI, FZK_IMARCH, FZK_IPSI, FZK_INHAT, FZK_IFLUX, FZK_TEMP, FZK_MOM, FZK_FFTX_FWD,
-                  FZK_SPEC_FWD, FZK_SPEC_BWD, FZK_FFTX_INV, FZK_CORRECT, FZK_OTHER, FZK_COUNT };
+                  FZK_SPEC_FWD, FZK_SPEC_BWD, FZK_FFTX_INV, FZK_CORRECT, FZK_OTHER, FZK_MG, FZK_COUNT };
 static const char *const FZK_NAME[FZK_COUNT] = {
     "k_latch_gamma", "k_phi_update", "k_corr_phi", "k_iface_march", "k_iface_psi", "k_iface_nhat", "k_iface_flux", "k_temp_update", "k_momentum",
-    "k_fftx_fwd", "k_spec_fwd", "k_spec_bwd", "k_fftx_inv", "k_correct", "other"};
+    "k_fftx_fwd", "k_spec_fwd", "k_spec_bwd", "k_fftx_inv", "k_correct", "other", "mg_cg_solve (whole call)"};
 
 struct FzTimed { int id; cudaEvent_t e0, e1; };
 
@@ -406,6 +406,7 @@ extern "C" fizzy_status fizzy_timing_get(fizzy_ctx *c, int index, const char **n
         for (FzTimed &t : c->pending) {
             float ms = 0.f;
             if (t.e0 && t.e1 && cudaEventElapsedTime(&ms, t.e0, t.e1) == cudaSuccess) { c->t_ms[t.id] += ms; ++c->t_n[t.id]; }
+            else cudaGetLastError();   // e.g. an end event never recorded because its call failed midway: not a launch error
             if (t.e0) c->pool.push_back(t.e0);
             if (t.e1) c->pool.push_back(t.e1);
         }
@@ -418,6 +419,7 @@ extern "C" fizzy_status fizzy_timing_get(fizzy_ctx *c, int index, const char **n
     return FIZZY_OK;
 }
 
+extern "C" int fizzy_abi_version(void) { return FIZZY_ABI_VERSION; }
 extern "C" const char *fizzy_last_error(const fizzy_ctx *c) { return c ? c->err.c_str() : "null context"; }
 extern "C" long long fizzy_launch_count(const fizzy_ctx *c) { return c ? c->launches : 0; }
 
@@ -954,6 +956,10 @@ extern "C" fizzy_status fizzy_poisson_solve_varcoef(fizzy_ctx *c, const double *
     const FzP &P = c->P;
     const int n = (int)c->N;
     cudaStream_t st = c->stream;
+    // timing mode: ONE event pair around the whole solve (its kernels are launched from lambdas, outside FZ_TB); the
+    // time includes the host round trips of the CG scalars
+    FZ_TB(FZK_MG);
+    const size_t mg_slot = c->pending.size();   // 0 when timing is off
     Carver cv(dev_work);
     double *sol = cv.dbl(n), *res = cv.dbl(n), *dir = cv.dbl(n), *q = cv.dbl(n);
     FzMgLevel L[FZ_MG_MAXLEV];
@@ -969,11 +975,15 @@ extern "C" fizzy_status fizzy_poisson_solve_varcoef(fizzy_ctx *c, const double *
         L[l].bx = cv.dbl(nl); L[l].by = cv.dbl(nl); L[l].bz = cv.dbl(nl);
     }
     // 1-D z tables of every level: dzf (sum of the two children), centre spacings from face midpoints (N10)
+    // (all levels in one host vector: one copy and one synchronisation instead of one per level)
     std::vector<double> dz = c->hdzf;
+    size_t tab_off[FZ_MG_MAXLEV], tab_len = 0;
+    for (int l = 0; l < plan.nlev; ++l) { tab_off[l] = tab_len; tab_len += (3 * (size_t)plan.nz[l] + 31) & ~size_t(31); }   // 256-byte pieces
+    tab.assign(tab_len, 0.0);
     for (int l = 0; l < plan.nlev; ++l) {
         const int nzl = plan.nz[l];
         if (l > 0) { std::vector<double> cz(nzl); for (int k = 0; k < nzl; ++k) cz[k] = dz[2 * k] + dz[2 * k + 1]; dz.swap(cz); }
-        std::vector<double> t(3 * (size_t)nzl);
+        double *t = tab.data() + tab_off[l];
         for (int k = 0; k < nzl; ++k) {
             const int kp = k + 1 == nzl ? 0 : k + 1, km = k == 0 ? nzl - 1 : k - 1;
             const double dzc_p = 0.5 * (dz[k] + dz[kp]), dzc_m = 0.5 * (dz[km] + dz[k]);
@@ -981,10 +991,15 @@ extern "C" fizzy_status fizzy_poisson_solve_varcoef(fizzy_ctx *c, const double *
             t[nzl + k] = (P.z_wall && k == nzl - 1) ? 0.0 : 1.0 / (dzc_p * dz[k]);
             t[2 * nzl + k] = (P.z_wall && k == 0) ? 0.0 : 1.0 / (dzc_m * dz[k]);
         }
-        double *dt = cv.dbl(3 * (size_t)nzl);
-        FZ_CUDA(cudaMemcpyAsync(dt, t.data(), t.size() * sizeof(double), cudaMemcpyHostToDevice, st));
-        FZ_CUDA(cudaStreamSynchronize(st));   // t goes out of scope
-        L[l].wz = dt; L[l].czh = dt + nzl; L[l].czl = dt + 2 * nzl;
+    }
+    {
+        double *dt = cv.dbl(tab_len);
+        FZ_CUDA(cudaMemcpyAsync(dt, tab.data(), tab_len * sizeof(double), cudaMemcpyHostToDevice, st));
+        FZ_CUDA(cudaStreamSynchronize(st));   // pageable source: the copy has left the host vector
+        for (int l = 0; l < plan.nlev; ++l) {
+            const int nzl = plan.nz[l];
+            L[l].wz = dt + tab_off[l]; L[l].czh = L[l].wz + nzl; L[l].czl = L[l].wz + 2 * nzl;
+        }
     }
     double *partial = cv.dbl(FZ_MG_RBLOCKS), *scalar = cv.dbl(8);
     dim3 grid, block;
@@ -1097,6 +1112,7 @@ extern "C" fizzy_status fizzy_poisson_solve_varcoef(fizzy_ctx *c, const double *
     ++c->launches;
     FZ_CUDA(cudaPeekAtLastError());
     FZ_CUDA(cudaMemcpyAsync(p, sol, (size_t)n * sizeof(double), cudaMemcpyDefault, st));
+    if (c->timing && mg_slot && c->pending[mg_slot - 1].e1) cudaEventRecord(c->pending[mg_slot - 1].e1, st);
     if (iters) *iters = it;
     if (relres) *relres = bb > 0.0 ? std::sqrt(rr / bb) : 0.0;
     return FIZZY_OK;

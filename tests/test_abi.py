@@ -35,6 +35,12 @@ def test_header_symbols_are_exported(binding):
         assert hasattr(lib, n), n
 
 
+def test_abi_version_matches_the_header(binding):
+    text = open(os.path.join(ROOT, "include", "fizzy.h")).read()
+    declared = int(re.search(r"#define\s+FIZZY_ABI_VERSION\s+(\d+)", text).group(1))
+    assert binding._lib.fizzy_abi_version() == declared == binding.FIZZY_ABI_VERSION
+
+
 def test_only_sm100a_code_in_the_library(binding):
     import subprocess
     out = subprocess.run(["/usr/local/cuda/bin/cuobjdump", "-lelf", binding.LIB_PATH], capture_output=True, text=True).stdout
